@@ -1,0 +1,25 @@
+"""Builds oracle/libhomg_oracle.so from oracle/homg_oracle.cpp with g++.
+
+ORACLE = TEST INFRASTRUCTURE.  Called by tests/conftest.py, __graft_entry__.build()
+and bench.py's cpu_baseline / --impl reference legs; never by the product path.
+"""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "homg_oracle.cpp")
+LIB = os.path.join(HERE, "libhomg_oracle.so")
+
+# -ffp-contract=off: the oracle's arithmetic is exactly the expression tree written
+# in the source (no fused multiply-adds), so a reader can check it by eye.
+CMD = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-ffp-contract=off", "-o", LIB, SRC]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
+        subprocess.check_call(CMD)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))
