@@ -1,0 +1,152 @@
+/* homg.h — C ABI of libhomg.so: the high-occupancy multigrid (HOMG) cycle of
+ * arxiv 1108.2045 on one B200 (sm_100a).
+ *
+ * The library solves  A u = f  (Eq.1) with  A = -div(k grad)  on a
+ * nested hierarchy of structured grids with Dirichlet u = 0 (Eq.4;
+ * the paper writes lap u = f, its f is minus ours — DESIGN.md R1).  One call of
+ * homg_cycle runs outer HOMG cycles entirely on the device: residual (L75),
+ * nested full-weighting restriction of the residual to every level (L47, L67, L73),
+ * the MFMG schedule of whole-level iterations in which the interpolation of the
+ * coarse variations and the damped-Jacobi relaxation are one task (L51, L53-71),
+ * and the correction u += e (L75).  No host<->device transfer happens inside
+ * homg_cycle.
+ *
+ * Conventions
+ *   - dims[a] = nodes per axis INCLUDING the two Dirichlet boundary nodes, dims[0]
+ *     slowest (C order).  ndim = 2: (ny, nx); ndim = 3: (nz, ny, nx).
+ *   - every dims[a] must equal c_a * 2^(levels-1) + 1 with c_a >= 2.
+ *   - level m = 0 is the finest; level m has (dims[a]-1)/2^m + 1 nodes per axis and
+ *     mesh width h_m = 2^m h.
+ *   - user arrays (f, u0, k, solution) are DENSE C-order arrays of prod(dims) scalars
+ *     of the solver's dtype.  Boundary entries of f and u0 are ignored; the
+ *     solution has zeros there.
+ *   - "on_device" != 0: the pointer is a CUDA device pointer; 0: a host pointer
+ *     (the call then performs the H2D / D2H copy itself, synchronously).
+ *   - ownership: the caller owns the workspace and every in/out buffer; the library
+ *     owns only its host-side object, CUDA graphs and a few bytes of pinned memory.
+ *   - errors: every call returns a homg_status; nothing throws or aborts.  The text
+ *     of the last error is available from homg_last_error.
+ *   - all device work is issued on the stream given in homg_options.cuda_stream
+ *     (NULL = the legacy default stream).
+ */
+#ifndef HOMG_H_
+#define HOMG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define HOMG_API __attribute__((visibility("default")))
+#else
+#define HOMG_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct homg_solver homg_solver; /* opaque */
+
+typedef enum {
+    HOMG_OK = 0,
+    HOMG_EINVAL = 1, /* bad argument (dims/levels mismatch, null pointer, bad schedule) */
+    HOMG_ENOMEM = 2, /* workspace too small / host allocation failed               */
+    HOMG_ECUDA = 3,  /* a CUDA call failed; see homg_last_error                   */
+    HOMG_ESTATE = 4  /* call out of order (cycle before set_rhs, ...)             */
+} homg_status;
+
+typedef enum { HOMG_F32 = 4, HOMG_F64 = 8 } homg_dtype;
+
+typedef enum {
+    HOMG_POISSON5 = 0,  /* 2-D, 5-point  -lap                     (Eq.3) */
+    HOMG_POISSON7 = 1,  /* 3-D, 7-point  -lap                     (R10)        */
+    HOMG_DIFFUSION7 = 2 /* 3-D, 7-point  -div(k grad), nodal k,
+                           harmonic-mean faces, rediscretised per level (R11)  */
+} homg_stencil;
+
+/* MFMG schedule kinds (Fig.1 is missing — DESIGN.md R3).
+ * its(m) = min(2^(M-m+1), max_iters), M = levels-1. */
+enum {
+    HOMG_SCHED_C = 0,        /* M, then for k=M-1..0: k, and if k>0: k+1   (default) */
+    HOMG_SCHED_A = 1,        /* M, M-1, then for k=M-2..0: k+2, k+1, k               */
+    HOMG_SCHED_SAWTOOTH = 2, /* for k=M..0: M, M-1, .., k                            */
+    HOMG_SCHED_EXPLICIT = 3  /* sched_levels / sched_iters, must end on level 0      */
+};
+
+typedef struct {
+    double omega;     /* weighted-Jacobi damping; <= 0: 4/5 (2-D), 6/7 (3-D)             */
+    double h;         /* fine mesh width; <= 0: 1/(dims[0]-1)                            */
+    int max_iters;    /* MaxI; <= 0: 4                                    */
+    int schedule;     /* HOMG_SCHED_*                                                    */
+    const int* sched_levels; /* HOMG_SCHED_EXPLICIT: level of every visit (host ptr)     */
+    const int* sched_iters;  /* HOMG_SCHED_EXPLICIT: iterations of every visit, >= 1     */
+    int sched_len;
+    int coarse_threshold_nodes; /* levels with <= this many nodes run inside the one
+                                   persistent coarse-level launch; <= 0: library default */
+    int use_graph;    /* 1 (default when < 0): replay one CUDA graph per cycle; 0: plain
+                         stream launches (debugging, profiling)                          */
+    int history_cap;  /* capacity of the device-side norm history; <= 0: 4096            */
+    void* cuda_stream; /* cudaStream_t; NULL = legacy default stream                     */
+} homg_options;
+
+/* Fills *opt with the defaults (all "use default" markers). */
+HOMG_API void homg_default_options(homg_options* opt);
+
+/* Bytes of device workspace homg_create needs for this hierarchy (0 on bad arguments).
+ * Layout: DESIGN.md "Data layout in HBM" — every level array is contiguous, rows padded
+ * to a multiple of 128 bytes, every array 256-byte aligned. */
+HOMG_API size_t homg_workspace_bytes(int ndim, const int64_t* dims, int levels, homg_stencil stencil,
+                            homg_dtype dtype);
+
+/* Creates a solver over caller-owned device memory [workspace_dev, +workspace_bytes).
+ * The workspace is zeroed.  opt may be NULL.  PAPER.md L41-45 (problem), L67 (levels),
+ * L69-71 (schedule). */
+HOMG_API homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int levels,
+                        homg_stencil stencil, homg_dtype dtype, void* workspace_dev,
+                        size_t workspace_bytes, const homg_options* opt);
+
+/* Right-hand side f (Eq.1).  Resets the norm history. */
+HOMG_API homg_status homg_set_rhs(homg_solver* s, const void* f, int on_device);
+
+/* Initial guess u0 (default 0).  Resets the norm history. */
+HOMG_API homg_status homg_set_initial_guess(homg_solver* s, const void* u0, int on_device);
+
+/* Nodal coefficient k > 0 (HOMG_DIFFUSION7 only): sampled onto every level by
+ * injection (R11).  Must be called before homg_cycle for that stencil. */
+HOMG_API homg_status homg_set_coefficient(homg_solver* s, const void* k, int on_device);
+
+/* n outer cycles (residual -> restrict -> MFMG -> u += e), asynchronous on
+ * the solver's stream, no host transfers.  Appends n entries to the norm history:
+ * entry c = || f - A u ||_2 BEFORE cycle c (sum over interior nodes, accumulated in
+ * fp64, no h^d factor — DESIGN.md R12). */
+HOMG_API homg_status homg_cycle(homg_solver* s, int n);
+
+/* || f - A u ||_2 of the CURRENT u (one norm-only pass, stream sync, 8-byte D2H) and its
+ * ratio to the first history entry (the norm of the initial guess; 1 if no cycle ran).
+ * Either output pointer may be NULL. */
+HOMG_API homg_status homg_residual_norm(homg_solver* s, double* abs_l2, double* rel_to_initial);
+
+/* Copies min(cap, count) history entries (L2 norms, not squared) to host `out`; syncs. */
+HOMG_API homg_status homg_residual_history(homg_solver* s, double* out, int cap, int* count);
+
+/* Dense C-order copy of u (boundary = 0) into dst; syncs when dst is a host pointer. */
+HOMG_API homg_status homg_get_solution(homg_solver* s, void* dst, int on_device);
+
+/* Introspection for tests and the bench harness: the effective schedule (returns its
+ * length; copies at most cap entries), the number of kernel launches one cycle issues,
+ * and the algorithmic HBM bytes one cycle moves on level 0 / on all levels
+ * (DESIGN.md "Roofline"). */
+HOMG_API int homg_get_schedule(const homg_solver* s, int* levels_out, int* iters_out, int cap);
+HOMG_API int homg_launches_per_cycle(const homg_solver* s);
+HOMG_API double homg_bytes_per_cycle(const homg_solver* s, int level0_only);
+
+HOMG_API void homg_destroy(homg_solver* s);
+
+/* Text of the last error on this solver ("" if none).  s may be NULL: returns the text
+ * of the last homg_create failure on this thread. */
+HOMG_API const char* homg_last_error(const homg_solver* s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOMG_H_ */

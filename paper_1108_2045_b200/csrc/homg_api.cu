@@ -1,0 +1,264 @@
+// homg_api.cu — the C ABI of libhomg.so (include/homg.h): argument checking, workspace carving,
+// graph capture and replay.  No arithmetic of the method happens on the host.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "homg_exec.h"
+
+using namespace homg;
+
+namespace {
+
+thread_local std::string g_create_err;
+
+size_t round_up(size_t v, size_t m) { return (v + m - 1) / m * m; }
+
+homg_status set_err(homg_solver* s, homg_status st, const std::string& msg) {
+    if (s) s->err = msg; else g_create_err = msg;
+    return st;
+}
+
+homg_status cuda_fail(homg_solver* s, cudaError_t e, const char* where) {
+    return set_err(s, HOMG_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(s, call)                                                    \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return cuda_fail((s), e__, #call);     \
+    } while (0)
+
+void drop_graph(homg_solver* s) {
+    if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+    if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+}
+
+homg_status reset_history(homg_solver* s) {
+    CU(s, cudaMemsetAsync(s->slot, 0, sizeof(int), s->stream));
+    s->cycles_issued = 0;
+    return HOMG_OK;
+}
+
+// copies a user array (host or device, dense) into a padded level-0 array
+homg_status load_dense(homg_solver* s, const void* src, int on_device, void* padded, int zero_boundary) {
+    const LevelGeom& g = s->L[0].g;
+    size_t bytes = size_t(g.nx) * g.ny * g.nz * size_t(s->dtype);
+    const void* dense = src;
+    if (!on_device) {
+        CU(s, cudaMemcpyAsync(s->staging, src, bytes, cudaMemcpyHostToDevice, s->stream));
+        dense = s->staging;
+    }
+    CU(s, exec_pack(s, s->stream, dense, padded, zero_boundary));
+    if (!on_device) CU(s, cudaStreamSynchronize(s->stream));   // the host buffer may be reused on return
+    return HOMG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void homg_default_options(homg_options* o) {
+    if (!o) return;
+    std::memset(o, 0, sizeof(*o));
+    o->omega = 0; o->h = 0; o->max_iters = 0; o->schedule = HOMG_SCHED_C;
+    o->coarse_threshold_nodes = 0; o->use_graph = -1; o->history_cap = 0; o->cuda_stream = nullptr;
+}
+
+size_t homg_workspace_bytes(int ndim, const int64_t* dims, int levels, homg_stencil st, homg_dtype dt) {
+    Plan P;
+    if (!plan_layout(ndim, dims, levels, st, dt, P, &g_create_err)) return 0;
+    return P.total_bytes + round_up(size_t(4096) * sizeof(double), 256);   // default history
+}
+
+homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int levels, homg_stencil st,
+                        homg_dtype dt, void* ws, size_t ws_bytes, const homg_options* opt) {
+    if (!out) return set_err(nullptr, HOMG_EINVAL, "out is null");
+    *out = nullptr;
+    Plan P;
+    std::string why;
+    if (!plan_layout(ndim, dims, levels, st, dt, P, &why)) return set_err(nullptr, HOMG_EINVAL, why);
+    if (!ws) return set_err(nullptr, HOMG_EINVAL, "workspace is null");
+    homg_options o;
+    homg_default_options(&o);
+    if (opt) o = *opt;
+    int hist_cap = o.history_cap > 0 ? o.history_cap : 4096;
+    size_t need = P.total_bytes + round_up(size_t(hist_cap) * sizeof(double), 256);
+    if (ws_bytes < need) return set_err(nullptr, HOMG_ENOMEM, "workspace too small (see homg_workspace_bytes)");
+    if ((reinterpret_cast<uintptr_t>(ws) & 255) != 0) return set_err(nullptr, HOMG_EINVAL, "workspace must be 256-byte aligned");
+
+    homg_solver* s = new (std::nothrow) homg_solver();
+    if (!s) return set_err(nullptr, HOMG_ENOMEM, "host allocation failed");
+    s->ndim = ndim; s->levels = levels; s->stencil = st; s->dtype = dt; s->var = P.var;
+    s->omega = o.omega > 0 ? o.omega : (ndim == 2 ? 4.0 / 5.0 : 6.0 / 7.0);
+    s->h = o.h > 0 ? o.h : 1.0 / double(dims[0] - 1);
+    s->max_iters = o.max_iters > 0 ? o.max_iters : 4;
+    s->coarse_threshold = o.coarse_threshold_nodes;
+    s->use_graph = o.use_graph != 0;
+    s->stream = static_cast<cudaStream_t>(o.cuda_stream);
+    s->hist_cap = hist_cap;
+    if (build_schedule(o.schedule, levels, s->max_iters, o.sched_levels, o.sched_iters, o.sched_len, s->sched_lv,
+                       s->sched_it, &why) < 0) {
+        delete s;
+        return set_err(nullptr, HOMG_EINVAL, why);
+    }
+    // ---- carve the workspace ----
+    s->ws_base = static_cast<char*>(ws); s->ws_bytes = ws_bytes;
+    char* p = s->ws_base + 256;             // front guard
+    size_t es = size_t(dt);
+    auto take = [&](size_t bytes) { void* r = p; p += round_up(bytes, 256); return r; };
+    s->L.resize(levels);
+    for (int m = 0; m < levels; ++m) {
+        Level& L = s->L[m];
+        L.g = P.g[m]; L.n_alloc = P.n_alloc[m];
+        L.n_nodes = (long long)L.g.nx * L.g.ny * L.g.nz;
+        L.h = s->h * double(1LL << m);
+        size_t ab = L.n_alloc * es;
+        L.nrot = (m == 0) ? 3 : kNumRot;
+        if (m == 0) { s->u = take(ab); s->f = take(ab); }
+        L.gsrc = take(ab);
+        for (int b = 0; b < L.nrot; ++b) L.rot[b] = take(ab);
+        if (m >= 1) { L.a = take(ab); L.d0 = take(ab); L.tmp = take(ab); }
+        if (P.var) L.k = take(ab);
+    }
+    s->staging = take(P.staging_bytes);
+    s->partial = static_cast<double*>(take(P.partial_count * sizeof(double)));
+    s->partial_count = P.partial_count;
+    s->hist = static_cast<double*>(take(size_t(hist_cap) * sizeof(double)));
+    s->slot = static_cast<int*>(take(256));
+    s->scalar = reinterpret_cast<double*>(reinterpret_cast<char*>(s->slot) + 128);
+    if (size_t(p - s->ws_base) > ws_bytes) { delete s; return set_err(nullptr, HOMG_ENOMEM, "internal: layout exceeds plan"); }
+
+    cudaError_t e = cudaMemsetAsync(ws, 0, size_t(p - s->ws_base), s->stream);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {
+        homg_status r = cuda_fail(nullptr, e, "homg_create");
+        delete s;
+        return r;
+    }
+    *out = s;
+    return HOMG_OK;
+}
+
+homg_status homg_set_rhs(homg_solver* s, const void* f, int on_device) {
+    if (!s) return HOMG_EINVAL;
+    if (!f) return set_err(s, HOMG_EINVAL, "f is null");
+    homg_status r = load_dense(s, f, on_device, s->f, 1);
+    if (r != HOMG_OK) return r;
+    s->have_rhs = true;
+    return reset_history(s);
+}
+
+homg_status homg_set_initial_guess(homg_solver* s, const void* u0, int on_device) {
+    if (!s) return HOMG_EINVAL;
+    if (!u0) return set_err(s, HOMG_EINVAL, "u0 is null");
+    homg_status r = load_dense(s, u0, on_device, s->u, 1);
+    if (r != HOMG_OK) return r;
+    return reset_history(s);
+}
+
+homg_status homg_set_coefficient(homg_solver* s, const void* k, int on_device) {
+    if (!s) return HOMG_EINVAL;
+    if (!s->var) return set_err(s, HOMG_EINVAL, "this stencil has no coefficient");
+    if (!k) return set_err(s, HOMG_EINVAL, "k is null");
+    homg_status r = load_dense(s, k, on_device, s->L[0].k, 0);
+    if (r != HOMG_OK) return r;
+    CU(s, exec_sample_coef(s, s->stream));
+    s->have_coef = true;
+    return reset_history(s);
+}
+
+homg_status homg_cycle(homg_solver* s, int n) {
+    if (!s) return HOMG_EINVAL;
+    if (n < 0) return set_err(s, HOMG_EINVAL, "n < 0");
+    if (!s->have_rhs) return set_err(s, HOMG_ESTATE, "homg_cycle before homg_set_rhs");
+    if (s->var && !s->have_coef) return set_err(s, HOMG_ESTATE, "homg_cycle before homg_set_coefficient");
+    if (s->use_graph && !s->graph_exec) {
+        // capture one cycle on the private stream (capturing does not execute anything)
+        CU(s, cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+        cudaError_t e = exec_cycle(s, s->cap_stream);
+        cudaError_t e2 = cudaStreamEndCapture(s->cap_stream, &s->graph);
+        if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "capture(exec_cycle)"); }
+        if (e2 != cudaSuccess) { drop_graph(s); return cuda_fail(s, e2, "cudaStreamEndCapture"); }
+        e = cudaGraphInstantiate(&s->graph_exec, s->graph, 0);
+        if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "cudaGraphInstantiate"); }
+    }
+    for (int i = 0; i < n; ++i) {
+        if (s->use_graph) CU(s, cudaGraphLaunch(s->graph_exec, s->stream));
+        else CU(s, exec_cycle(s, s->stream));
+    }
+    s->cycles_issued += n;
+    return HOMG_OK;
+}
+
+homg_status homg_residual_norm(homg_solver* s, double* abs_l2, double* rel) {
+    if (!s) return HOMG_EINVAL;
+    if (!s->have_rhs) return set_err(s, HOMG_ESTATE, "homg_residual_norm before homg_set_rhs");
+    CU(s, exec_norm_only(s, s->stream));
+    double n2 = 0, first2 = 0;
+    CU(s, cudaMemcpyAsync(&n2, s->scalar, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    if (rel && s->cycles_issued > 0)
+        CU(s, cudaMemcpyAsync(&first2, s->hist, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    double nn = std::sqrt(n2);
+    if (abs_l2) *abs_l2 = nn;
+    if (rel) *rel = (s->cycles_issued > 0 && first2 > 0) ? nn / std::sqrt(first2) : 1.0;
+    return HOMG_OK;
+}
+
+homg_status homg_residual_history(homg_solver* s, double* out, int cap, int* count) {
+    if (!s) return HOMG_EINVAL;
+    long have = s->cycles_issued < s->hist_cap ? s->cycles_issued : s->hist_cap;
+    if (count) *count = int(have);
+    int n = int(have < cap ? have : cap);
+    if (out && n > 0) {
+        CU(s, cudaMemcpyAsync(out, s->hist, size_t(n) * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        CU(s, cudaStreamSynchronize(s->stream));
+        for (int i = 0; i < n; ++i) out[i] = std::sqrt(out[i]);
+    }
+    return HOMG_OK;
+}
+
+homg_status homg_get_solution(homg_solver* s, void* dst, int on_device) {
+    if (!s) return HOMG_EINVAL;
+    if (!dst) return set_err(s, HOMG_EINVAL, "dst is null");
+    const LevelGeom& g = s->L[0].g;
+    size_t bytes = size_t(g.nx) * g.ny * g.nz * size_t(s->dtype);
+    if (on_device) {
+        CU(s, exec_unpack(s, s->stream, s->u, dst));
+    } else {
+        CU(s, exec_unpack(s, s->stream, s->u, s->staging));
+        CU(s, cudaMemcpyAsync(dst, s->staging, bytes, cudaMemcpyDeviceToHost, s->stream));
+        CU(s, cudaStreamSynchronize(s->stream));
+    }
+    return HOMG_OK;
+}
+
+int homg_get_schedule(const homg_solver* s, int* lv, int* it, int cap) {
+    if (!s) return -1;
+    int n = int(s->sched_lv.size());
+    for (int i = 0; i < n && i < cap; ++i) {
+        if (lv) lv[i] = s->sched_lv[i];
+        if (it) it[i] = s->sched_it[i];
+    }
+    return n;
+}
+
+int homg_launches_per_cycle(const homg_solver* s) { return s ? s->launches_per_cycle : -1; }
+
+double homg_bytes_per_cycle(const homg_solver* s, int level0_only) {
+    if (!s) return -1.0;
+    return level0_only ? s->bytes_cycle_l0 : s->bytes_cycle_all;
+}
+
+void homg_destroy(homg_solver* s) {
+    if (!s) return;
+    drop_graph(s);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    delete s;
+}
+
+const char* homg_last_error(const homg_solver* s) { return s ? s->err.c_str() : g_create_err.c_str(); }
+
+}  // extern "C"

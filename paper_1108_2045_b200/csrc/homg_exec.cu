@@ -1,0 +1,259 @@
+// homg_exec.cu — the cycle executor: turns the schedule table into the launch sequence of one
+// outer HOMG cycle (Algorithm H), issued on a stream (captured once into a CUDA graph
+// by homg_api.cu).  Host logic only decides pointers and flags; every arithmetic step is a kernel.
+#include "homg_exec.h"
+
+#include "homg_kernels.cuh"
+
+namespace homg {
+
+namespace {
+
+struct Rec {                 // bookkeeping while recording
+    homg_solver* s;
+    cudaStream_t st;
+    cudaError_t err = cudaSuccess;
+    int launches = 0;
+    double bytes_all = 0, bytes_l0 = 0;
+    void check() {
+        cudaError_t e = cudaPeekAtLastError();
+        if (err == cudaSuccess && e != cudaSuccess) err = e;
+        ++launches;
+    }
+    void acct(int level, double arrays) {     // `arrays` passes over one level-`level` array
+        double b = arrays * double(s->L[level].n_nodes) * double(s->dtype);
+        bytes_all += b;
+        if (level == 0) bytes_l0 += b;
+    }
+};
+
+inline dim3 blk() { return dim3(32, 8, 1); }
+inline dim3 grd(const LevelGeom& g) { return dim3((g.nx + 31) / 32, (g.ny + 7) / 8, g.nz); }
+
+template <class T>
+Coef<T> make_coef(const homg_solver* s, int m) {
+    Coef<T> c;
+    double h = s->L[m].h;
+    c.ih2 = T(1.0 / (h * h));
+    c.w = T(s->omega);
+    c.twod = T(2 * s->ndim);
+    c.w_over_D = c.w / (c.twod * c.ih2);
+    return c;
+}
+
+template <class T>
+T* rotp(Level& L, int i) { return i < 0 ? nullptr : static_cast<T*>(L.rot[i]); }
+
+template <class T, int ND, bool VAR>
+void rec_norm(Rec& R, bool write_r, bool to_history) {
+    homg_solver* s = R.s;
+    Level& L0 = s->L[0];
+    dim3 g = grd(L0.g);
+    k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
+                                                   (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
+    R.check();
+    R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
+    int n = int(g.x * g.y * g.z);
+    k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
+                                        to_history ? 1 : 0, to_history ? nullptr : s->scalar);
+    R.check();
+}
+
+template <class T, int ND, bool VAR>
+void rec_cycle(Rec& R) {
+    homg_solver* s = R.s;
+    const int M = s->levels - 1;
+    std::vector<Level>& L = s->L;
+    for (auto& l : L) { l.e = 0; l.touched = false; l.vk = l.vkm1 = l.vkm2 = -1; l.eta_last = 0; }
+    std::vector<char> a_zero(s->levels, 1);      // a_m == 0 (nothing pending)
+    std::vector<char> dp_is_d0(s->levels, 0);    // eta == 1 visit: its dp is its own d0
+
+    // S1: r = f - A u, ||r||^2 -> history
+    rec_norm<T, ND, VAR>(R, true, true);
+    // S2: nested restriction g_m = P g_{m-1}
+    for (int m = 1; m <= M; ++m) {
+        k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
+        R.check();
+        R.acct(m - 1, 1.0); R.acct(m, 1.0);
+    }
+    // S3: MFMG visits
+    int cur = -1;
+    const int nv = int(s->sched_lv.size());
+    for (int vi = 0; vi < nv; ++vi) {
+        const int t = s->sched_lv[vi], eta = s->sched_it[vi];
+        Level& Lt = L[t];
+        bool have_d0 = false;
+        if (cur < 0) {
+            cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
+            R.check();
+            Lt.touched = true;
+        } else {
+            if (t < cur) {
+                // S3a deliver (interpolate + correct) level m -> m-1
+                for (int m = cur; m > t; --m) {
+                    Level& Lc = L[m];
+                    Level& Lf = L[m - 1];
+                    int ef_assign = Lf.touched ? 0 : 1;
+                    int af_mode = (m - 1 >= 1) ? (a_zero[m - 1] ? 2 : 1) : 0;
+                    const T* ac = a_zero[m] ? nullptr : (const T*)Lc.a;
+                    if (af_mode == 2 && !ac) af_mode = 0;          // 0 + 0: a stays "known zero"
+                    k_deliver<T, ND><<<grd(Lf.g), blk(), 0, R.st>>>(Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
+                                                                     rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
+                    R.check();
+                    R.acct(m, ac ? 2.0 : 1.0);
+                    R.acct(m - 1, (ef_assign ? 1.0 : 2.0) + (af_mode == 1 ? 2.0 : af_mode == 2 ? 1.0 : 0.0));
+                    Lf.touched = true;
+                    if (af_mode) a_zero[m - 1] = 0;
+                    a_zero[m] = 1;                                  // a_m delivered
+                }
+            } else if (t > cur) {
+                // S3b inject level m-1 -> m (same memory cells in the paper's single array)
+                for (int m = cur + 1; m <= t; ++m) {
+                    k_inject<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
+                                                                      rotp<T>(L[m], L[m].e));
+                    R.check();
+                    R.acct(m, 2.0);
+                    L[m].touched = true;
+                }
+            }
+            // S3c carried variation d0 on level t (not needed on level 0: a_0 does not exist)
+            if (t >= 1) {
+                Level& Lv = L[cur];
+                const T* X = rotp<T>(Lv, Lv.vk);
+                const T* Y = rotp<T>(Lv, Lv.vkm1);
+                if (t >= cur) {
+                    k_d0_up<T, ND><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
+                    R.check();
+                    R.acct(t, 3.0);
+                } else {
+                    const T* A = dp_is_d0[cur] ? (const T*)Lv.d0 : rotp<T>(Lv, Lv.vkm1);
+                    const T* B = dp_is_d0[cur] ? nullptr : rotp<T>(Lv, Lv.vkm2);
+                    for (int m = cur; m > t; --m) {
+                        bool last = (m - 1 == t);
+                        T* out = last ? (T*)Lt.d0 : (T*)L[m - 1].tmp;
+                        k_d0_down<T, ND><<<grd(L[m - 1].g), blk(), 0, R.st>>>(L[m - 1].g, L[m].g, A, B, out,
+                                                                               last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
+                        R.check();
+                        R.acct(m, B ? 2.0 : 1.0); R.acct(m - 1, 1.0);
+                        A = out; B = nullptr;
+                    }
+                }
+                have_d0 = true;
+            }
+        }
+        if (t >= 1 && !have_d0 && eta == 1) {        // first visit with eta = 1: its dp is d0 = 0
+            cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st);
+            R.check();
+            have_d0 = true;
+        }
+        // S3d eta damped-Jacobi sweeps; S3e bookkeeping fused into the last one; S4 u += e fused
+        // into the last sweep of the cycle.
+        const int v0 = Lt.e;
+        int in = v0, prev_in = -1, prev2 = -1;
+        Coef<T> cf = make_coef<T>(s, t);
+        for (int it = 0; it < eta; ++it) {
+            int out = -1;
+            for (int b = 0; b < Lt.nrot; ++b)
+                if (b != in && b != prev_in && !(t >= 1 && b == v0)) { out = b; break; }
+            bool last = (it == eta - 1);
+            bool book = last && t >= 1;
+            bool addu = last && vi == nv - 1;
+            k_relax<T, ND, VAR><<<grd(Lt.g), blk(), 0, R.st>>>(
+                Lt.g, cf, rotp<T>(Lt, in), (const T*)Lt.gsrc, (const T*)Lt.k, rotp<T>(Lt, out),
+                book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0),
+                addu ? (T*)s->u : nullptr);
+            R.check();
+            R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
+                          (addu ? 2.0 : 0.0));
+            prev2 = prev_in; prev_in = in; in = out;
+        }
+        if (t >= 1) a_zero[t] = 0;
+        Lt.vk = in; Lt.vkm1 = prev_in; Lt.vkm2 = prev2; Lt.e = in; Lt.eta_last = eta;
+        dp_is_d0[t] = (eta == 1);
+        cur = t;
+    }
+}
+
+template <class T, int ND, bool VAR>
+void rec_sample(Rec& R) {
+    homg_solver* s = R.s;
+    for (int m = 1; m < s->levels; ++m) {
+        k_sample_coef<T, ND><<<grd(s->L[m].g), blk(), 0, R.st>>>(s->L[m].g, s->L[m - 1].g, (const T*)s->L[m - 1].k,
+                                                                   (T*)s->L[m].k);
+        R.check();
+    }
+}
+
+template <class T, int ND>
+void rec_pack(Rec& R, const void* dense, void* padded, int zero_boundary) {
+    const LevelGeom& g = R.s->L[0].g;
+    k_pack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)dense, (T*)padded, zero_boundary);
+    R.check();
+}
+
+template <class T, int ND>
+void rec_unpack(Rec& R, const void* padded, void* dense) {
+    const LevelGeom& g = R.s->L[0].g;
+    k_unpack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)padded, (T*)dense);
+    R.check();
+}
+
+// dispatch on (dtype, ndim, var)
+#define HOMG_DISPATCH(s, FN, ...)                                                            \
+    do {                                                                                     \
+        if ((s)->dtype == HOMG_F32) {                                                        \
+            if ((s)->ndim == 2) FN<float, 2, false>(__VA_ARGS__);                            \
+            else if ((s)->var) FN<float, 3, true>(__VA_ARGS__);                              \
+            else FN<float, 3, false>(__VA_ARGS__);                                           \
+        } else {                                                                             \
+            if ((s)->ndim == 2) FN<double, 2, false>(__VA_ARGS__);                           \
+            else if ((s)->var) FN<double, 3, true>(__VA_ARGS__);                             \
+            else FN<double, 3, false>(__VA_ARGS__);                                          \
+        }                                                                                    \
+    } while (0)
+
+#define HOMG_DISPATCH2(s, FN, ...)                                                           \
+    do {                                                                                     \
+        if ((s)->dtype == HOMG_F32) {                                                        \
+            if ((s)->ndim == 2) FN<float, 2>(__VA_ARGS__); else FN<float, 3>(__VA_ARGS__);   \
+        } else {                                                                             \
+            if ((s)->ndim == 2) FN<double, 2>(__VA_ARGS__); else FN<double, 3>(__VA_ARGS__); \
+        }                                                                                    \
+    } while (0)
+
+}  // namespace
+
+cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
+    Rec R{s, st};
+    HOMG_DISPATCH(s, rec_cycle, R);
+    s->launches_per_cycle = R.launches;
+    s->bytes_cycle_all = R.bytes_all;
+    s->bytes_cycle_l0 = R.bytes_l0;
+    return R.err;
+}
+
+cudaError_t exec_norm_only(homg_solver* s, cudaStream_t st) {
+    Rec R{s, st};
+    HOMG_DISPATCH(s, rec_norm, R, false, false);
+    return R.err;
+}
+
+cudaError_t exec_sample_coef(homg_solver* s, cudaStream_t st) {
+    Rec R{s, st};
+    HOMG_DISPATCH(s, rec_sample, R);
+    return R.err;
+}
+
+cudaError_t exec_pack(homg_solver* s, cudaStream_t st, const void* dense_dev, void* padded, int zero_boundary) {
+    Rec R{s, st};
+    HOMG_DISPATCH2(s, rec_pack, R, dense_dev, padded, zero_boundary);
+    return R.err;
+}
+
+cudaError_t exec_unpack(homg_solver* s, cudaStream_t st, const void* padded, void* dense_dev) {
+    Rec R{s, st};
+    HOMG_DISPATCH2(s, rec_unpack, R, padded, dense_dev);
+    return R.err;
+}
+
+}  // namespace homg

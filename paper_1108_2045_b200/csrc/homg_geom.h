@@ -1,0 +1,20 @@
+// homg_geom.h — geometry of one level array, shared by host code and kernels.
+#pragma once
+
+namespace homg {
+
+struct LevelGeom {
+    int nx, ny, nz;      // nodes per axis incl. boundary (nz = 1 in 2-D)
+    int px;              // row pitch in elements
+    long long pp;        // plane pitch in elements (px*ny)
+};
+
+template <class T>
+struct Coef {            // per-level operator constants
+    T ih2;               // 1/h_m^2
+    T w;                 // omega
+    T w_over_D;          // omega / (2d/h_m^2)      (constant coefficient)
+    T twod;              // 2d
+};
+
+}  // namespace homg

@@ -1,0 +1,89 @@
+// homg_internal.h — host-side structures of libhomg.so (not installed; include/homg.h is the ABI).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/homg.h"
+#include "homg_geom.h"
+
+namespace homg {
+
+constexpr int kMaxLevels = 32;
+constexpr int kNumRot = 4;   // rotating correction buffers per level (v0, v^k, v^{k-1}, v^{k-2})
+
+// One level of the hierarchy.  All pointers are carved out of
+// the caller's workspace; every array holds n_alloc scalars.
+struct Level {
+    LevelGeom g;
+    size_t n_alloc = 0;        // scalars per array (pp*nz, rounded up so that bytes % 256 == 0, + pad)
+    long long n_nodes = 0;     // nx*ny*nz
+    double h = 0;              // mesh width 2^m h
+    void* rot[kNumRot] = {};   // correction buffers (level 0 uses 3)
+    int nrot = 0;
+    void* a = nullptr;         // pending increments (levels >= 1)
+    void* gsrc = nullptr;      // restricted residual g_m (level 0: the residual itself)
+    void* d0 = nullptr;        // carried variation (levels >= 1)
+    void* tmp = nullptr;       // scratch of the d0 prolongation chain (levels >= 1)
+    void* k = nullptr;         // nodal coefficient (HOMG_DIFFUSION7)
+    // --- executor state while one cycle is being recorded ---
+    int e = 0;                 // rot index holding the materialised correction e_m
+    bool touched = false;      // e_m / a_m already defined in this cycle
+    int vk = -1, vkm1 = -1, vkm2 = -1;   // rot indices of v^eta, v^{eta-1}, v^{eta-2} of the last visit
+    int eta_last = 0;
+};
+
+struct Plan {                  // result of plan_layout: sizes only, no pointers
+    int ndim = 0, levels = 0, esize = 0;
+    bool var = false;
+    std::vector<LevelGeom> g;
+    std::vector<size_t> n_alloc;
+    size_t staging_bytes = 0;  // dense level-0 array for pack/unpack
+    size_t partial_count = 0;  // doubles for per-block norm partials
+    size_t total_bytes = 0;
+};
+
+bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, homg_dtype dt, Plan& P,
+                 std::string* why);
+
+int build_schedule(int kind, int levels, int maxI, const int* xl, const int* xi, int xlen,
+                   std::vector<int>& lv, std::vector<int>& it, std::string* why);
+
+}  // namespace homg
+
+struct homg_solver {
+    int ndim = 0, levels = 0;
+    homg_stencil stencil = HOMG_POISSON5;
+    homg_dtype dtype = HOMG_F64;
+    bool var = false;
+    double omega = 0, h = 0;
+    int max_iters = 4;
+    int coarse_threshold = 0;
+    bool use_graph = true;
+    std::vector<int> sched_lv, sched_it;
+    std::vector<homg::Level> L;
+    // level-0 extras
+    void* u = nullptr;
+    void* f = nullptr;
+    void* staging = nullptr;
+    double* partial = nullptr;   // per-block partial sums of r^2
+    size_t partial_count = 0;
+    double* hist = nullptr;      // device norm^2 history
+    int hist_cap = 0;
+    int* slot = nullptr;         // device: next history slot
+    double* scalar = nullptr;    // device: result of a norm-only pass
+    char* ws_base = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;       // the caller's stream: all work is issued here
+    cudaStream_t cap_stream = nullptr;   // private stream used only to capture the graph
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    bool have_rhs = false, have_coef = false;
+    long cycles_issued = 0;
+    int launches_per_cycle = 0;
+    double bytes_cycle_all = 0, bytes_cycle_l0 = 0;
+    std::string err;
+};

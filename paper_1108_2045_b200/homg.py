@@ -1,0 +1,194 @@
+"""Thin ctypes binding of libhomg.so (include/homg.h).  Argument marshalling only: every step of
+the HOMG cycle runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream.
+
+There is NO CPU fallback: if libhomg.so is missing or cannot be loaded this module raises.
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libhomg.so")
+
+HOMG_OK, HOMG_EINVAL, HOMG_ENOMEM, HOMG_ECUDA, HOMG_ESTATE = range(5)
+HOMG_F32, HOMG_F64 = 4, 8
+HOMG_POISSON5, HOMG_POISSON7, HOMG_DIFFUSION7 = 0, 1, 2
+HOMG_SCHED_C, HOMG_SCHED_A, HOMG_SCHED_SAWTOOTH, HOMG_SCHED_EXPLICIT = 0, 1, 2, 3
+STENCILS = {"poisson5": HOMG_POISSON5, "poisson7": HOMG_POISSON7, "diffusion7": HOMG_DIFFUSION7}
+DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
+
+# every symbol include/homg.h declares (tests check that the library exports each one)
+SYMBOLS = [
+    "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
+    "homg_set_coefficient", "homg_cycle", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
+    "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
+]
+
+
+class HomgOptions(C.Structure):
+    _fields_ = [
+        ("omega", C.c_double), ("h", C.c_double), ("max_iters", C.c_int), ("schedule", C.c_int),
+        ("sched_levels", C.POINTER(C.c_int)), ("sched_iters", C.POINTER(C.c_int)), ("sched_len", C.c_int),
+        ("coarse_threshold_nodes", C.c_int), ("use_graph", C.c_int), ("history_cap", C.c_int),
+        ("cuda_stream", C.c_void_p),
+    ]
+
+
+class HomgError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"homg status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Loads libhomg.so (never builds, never falls back)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1108_2045_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, d = C.c_void_p, C.c_int, C.c_double
+        i64p = C.POINTER(C.c_int64)
+        L.homg_default_options.argtypes = [C.POINTER(HomgOptions)]; L.homg_default_options.restype = None
+        L.homg_workspace_bytes.argtypes = [i, i64p, i, i, i]; L.homg_workspace_bytes.restype = C.c_size_t
+        L.homg_create.argtypes = [C.POINTER(vp), i, i64p, i, i, i, vp, C.c_size_t, C.POINTER(HomgOptions)]
+        L.homg_create.restype = i
+        for name in ("homg_set_rhs", "homg_set_initial_guess", "homg_set_coefficient", "homg_get_solution"):
+            getattr(L, name).argtypes = [vp, vp, i]; getattr(L, name).restype = i
+        L.homg_cycle.argtypes = [vp, i]; L.homg_cycle.restype = i
+        L.homg_residual_norm.argtypes = [vp, C.POINTER(d), C.POINTER(d)]; L.homg_residual_norm.restype = i
+        L.homg_residual_history.argtypes = [vp, C.POINTER(d), i, C.POINTER(i)]; L.homg_residual_history.restype = i
+        L.homg_get_schedule.argtypes = [vp, C.POINTER(i), C.POINTER(i), i]; L.homg_get_schedule.restype = i
+        L.homg_launches_per_cycle.argtypes = [vp]; L.homg_launches_per_cycle.restype = i
+        L.homg_bytes_per_cycle.argtypes = [vp, i]; L.homg_bytes_per_cycle.restype = d
+        L.homg_destroy.argtypes = [vp]; L.homg_destroy.restype = None
+        L.homg_last_error.argtypes = [vp]; L.homg_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _dims(dims):
+    return (C.c_int64 * len(dims))(*[int(x) for x in dims])
+
+
+def workspace_bytes(dims, levels, stencil, dtype):
+    return int(lib().homg_workspace_bytes(len(dims), _dims(dims), levels, STENCILS[stencil], DTYPES[dtype]))
+
+
+def _ptr_and_flag(x):
+    """(pointer, on_device) of a torch tensor (CUDA or CPU) or a numpy array; must be C-contiguous."""
+    if hasattr(x, "data_ptr"):            # torch.Tensor
+        if not x.is_contiguous():
+            raise ValueError("array must be contiguous")
+        return x.data_ptr(), 1 if x.is_cuda else 0
+    if not x.flags["C_CONTIGUOUS"]:
+        raise ValueError("array must be C-contiguous")
+    return x.ctypes.data, 0
+
+
+class Solver:
+    """homg_create ... homg_destroy.  The workspace is a torch uint8 CUDA tensor owned by this object."""
+
+    def __init__(self, dims, levels, stencil, dtype, omega=0.0, h=0.0, max_iters=0, schedule=HOMG_SCHED_C,
+                 sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, device="cuda:0", stream=None):
+        import torch
+        self._torch = torch
+        self.dims = tuple(int(x) for x in dims)
+        self.levels = int(levels)
+        self.dtype = dtype
+        self.handle = C.c_void_p(None)
+        L = lib()
+        self.device = torch.device(device)
+        if self.device.type != "cuda":
+            raise ValueError("homg runs on a CUDA device only (no CPU fallback)")
+        o = HomgOptions()
+        L.homg_default_options(C.byref(o))
+        o.omega, o.h, o.max_iters, o.schedule = float(omega), float(h), int(max_iters), int(schedule)
+        o.coarse_threshold_nodes, o.use_graph, o.history_cap = int(coarse_threshold_nodes), int(use_graph), int(history_cap)
+        self._keep = None
+        if sched is not None:
+            lv, it = sched
+            a = (C.c_int * len(lv))(*lv); b = (C.c_int * len(it))(*it)
+            self._keep = (a, b)
+            o.schedule, o.sched_levels, o.sched_iters, o.sched_len = HOMG_SCHED_EXPLICIT, a, b, len(lv)
+        with torch.cuda.device(self.device):
+            st = stream if stream is not None else torch.cuda.current_stream(self.device)
+            o.cuda_stream = C.c_void_p(st.cuda_stream)
+            need = L.homg_workspace_bytes(len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil], DTYPES[dtype])
+            if need == 0:
+                raise HomgError(HOMG_EINVAL, L.homg_last_error(None).decode())
+            need += max(0, int(history_cap) - 4096) * 8 + 256
+            self.workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
+            rc = L.homg_create(C.byref(self.handle), len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil],
+                               DTYPES[dtype], C.c_void_p(self.workspace.data_ptr()), need, C.byref(o))
+        if rc != HOMG_OK:
+            self.handle = C.c_void_p(None)
+            raise HomgError(rc, L.homg_last_error(None).decode())
+
+    # -- helpers --
+    def _ck(self, rc):
+        if rc != HOMG_OK:
+            raise HomgError(rc, lib().homg_last_error(self.handle).decode())
+
+    def _call_arr(self, fn, x):
+        p, dev = _ptr_and_flag(x)
+        with self._torch.cuda.device(self.device):
+            self._ck(fn(self.handle, C.c_void_p(p), dev))
+
+    # -- the C-ABI calls, same names --
+    def set_rhs(self, f):
+        self._call_arr(lib().homg_set_rhs, f)
+
+    def set_initial_guess(self, u0):
+        self._call_arr(lib().homg_set_initial_guess, u0)
+
+    def set_coefficient(self, k):
+        self._call_arr(lib().homg_set_coefficient, k)
+
+    def cycle(self, n=1):
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().homg_cycle(self.handle, int(n)))
+
+    def residual_norm(self):
+        a = C.c_double(0); r = C.c_double(0)
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().homg_residual_norm(self.handle, C.byref(a), C.byref(r)))
+        return a.value, r.value
+
+    def residual_history(self):
+        n = C.c_int(0)
+        self._ck(lib().homg_residual_history(self.handle, None, 0, C.byref(n)))
+        buf = (C.c_double * max(1, n.value))()
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().homg_residual_history(self.handle, buf, n.value, C.byref(n)))
+        return list(buf[:n.value])
+
+    def get_solution(self, out):
+        self._call_arr(lib().homg_get_solution, out)
+        return out
+
+    def schedule(self):
+        n = lib().homg_get_schedule(self.handle, None, None, 0)
+        a = (C.c_int * n)(); b = (C.c_int * n)()
+        lib().homg_get_schedule(self.handle, a, b, n)
+        return list(a), list(b)
+
+    def launches_per_cycle(self):
+        return int(lib().homg_launches_per_cycle(self.handle))
+
+    def bytes_per_cycle(self, level0_only=False):
+        return float(lib().homg_bytes_per_cycle(self.handle, 1 if level0_only else 0))
+
+    def destroy(self):
+        if self.handle:
+            lib().homg_destroy(self.handle)
+            self.handle = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,201 @@
+"""-m gpu: parity of the CUDA path (through the C ABI, via the thin binding) against the oracle.
+
+Bar (BASELINE.json north_star / SURVEY.md 8(d)): after EVERY cycle
+    max|u_gpu - u_orc| / max|u_orc| <= 1e-12 (fp64) / 1e-5 (fp32, oracle also in fp32)
+and per-cycle residual factors equal to 3 significant digits while above the rounding floor.
+Inputs: paper_1108_2045_b200.inputs (seeded, synthetic; shared generator module, no arithmetic).
+"""
+import numpy as np
+import pytest
+
+from paper_1108_2045_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests")
+    return torch
+
+
+def run_gpu(cfg, inp, ncycles, **kw):
+    """Runs ncycles one at a time and returns (list of u after each cycle, norms[ncycles+1])."""
+    torch = _torch()
+    from paper_1108_2045_b200 import homg
+    s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters,
+                    schedule=cfg.schedule, **kw)
+    if inp["k"] is not None:
+        s.set_coefficient(inp["k"])
+    s.set_rhs(inp["f"])
+    s.set_initial_guess(inp["u0"])
+    us = []
+    out = np.empty(cfg.dims, dtype=cfg.np_dtype)
+    for _ in range(ncycles):
+        s.cycle(1)
+        us.append(s.get_solution(out).copy())
+    hist = s.residual_history()
+    final, rel = s.residual_norm()
+    assert len(hist) == ncycles
+    norms = np.array(hist + [final])
+    assert s.launches_per_cycle() > 0
+    sched = s.schedule()
+    s.destroy()
+    return us, norms, sched
+
+
+def check_parity(cfg, ncycles, orc, floor=None, **kw):
+    inp = I.make_inputs(cfg)
+    us, norms, sched = run_gpu(cfg, inp, ncycles, **kw)
+    osched = kw.get("sched") or orc.schedule(cfg.schedule, cfg.levels, cfg.max_iters)
+    assert (list(sched[0]), list(sched[1])) == (list(osched[0]), list(osched[1]))
+    _, hist, onorms = orc.homg("H", inp["f"], inp["u0"], cfg.levels, cfg.omega, osched, ncycles, k=inp["k"])
+    tol = TOL[cfg.dtype]
+    for c in range(ncycles):
+        ref = hist[c].astype(np.float64)
+        err = np.max(np.abs(us[c].astype(np.float64) - ref)) / np.max(np.abs(ref))
+        assert err <= tol, f"{cfg.name}: cycle {c}: max-norm relative difference {err:.3e} > {tol}"
+    # residual factors to 3 significant digits while above the floor
+    if floor is None:
+        floor = 1e-11 if cfg.dtype == "f64" else 3e-5
+    for c in range(1, ncycles + 1):
+        if onorms[c] / onorms[0] < floor:
+            break
+        fg, fo = norms[c] / norms[c - 1], onorms[c] / onorms[c - 1]
+        assert abs(fg - fo) <= 5e-3 * abs(fo) * (1 if cfg.dtype == "f32" else 0.2), (cfg.name, c, fg, fo)
+    return us, norms
+
+
+def test_cfg1_full(orc):
+    """BASELINE configs[0]: 129^2 fp64, 7 levels, 10 cycles, exactly as stated."""
+    cfg = I.CONFIGS["cfg1"]
+    us, norms = check_parity(cfg, 10, orc)
+    import os
+    golden = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "cfg1_norms.txt"), comments="#")
+    g = np.atleast_1d(golden).ravel()
+    n = min(len(g), len(norms))
+    assert np.allclose(norms[:n], g[:n], rtol=1e-9), "GPU norms differ from the oracle-written golden file"
+
+
+@pytest.mark.parametrize("n", [17, 33, 65])
+def test_cfg2_scaled(orc, n):
+    check_parity(I.scaled(I.CONFIGS["cfg2"], n), 6, orc)
+
+
+@pytest.mark.parametrize("n", [65, 257, 513])
+def test_cfg3_scaled(orc, n):
+    check_parity(I.scaled(I.CONFIGS["cfg3"], n), 5, orc)
+
+
+@pytest.mark.parametrize("n", [33, 65])
+def test_cfg4_scaled(orc, n):
+    check_parity(I.scaled(I.CONFIGS["cfg4"], n), 5, orc)
+
+
+@pytest.mark.parametrize("n", [17, 33, 65])
+def test_cfg5_scaled(orc, n):
+    check_parity(I.scaled(I.CONFIGS["cfg5"], n), 6, orc)
+
+
+@pytest.mark.parametrize("kind", [0, 1, 2])
+@pytest.mark.parametrize("maxi", [2, 4, 32])
+def test_schedules_2d(orc, kind, maxi):
+    import dataclasses
+    cfg = dataclasses.replace(I.scaled(I.CONFIGS["cfg1"], 65), schedule=kind, max_iters=maxi)
+    check_parity(cfg, 3, orc)
+
+
+@pytest.mark.parametrize("kind", [1, 2])
+def test_schedules_3d(orc, kind):
+    import dataclasses
+    cfg = dataclasses.replace(I.scaled(I.CONFIGS["cfg5"], 33), schedule=kind, max_iters=8)
+    check_parity(cfg, 3, orc)
+
+
+def test_explicit_schedule_with_single_iterations_and_fine_revisits(orc):
+    """eta = 1 visits, level 0 visited in mid-schedule, repeated level, multi-level jumps."""
+    cfg = I.scaled(I.CONFIGS["cfg1"], 33)
+    sched = ([4, 4, 2, 0, 3, 1, 1, 0, 2, 4, 0], [1, 2, 1, 2, 3, 1, 1, 1, 2, 2, 3])
+    check_parity(cfg, 3, orc, sched=sched)
+    cfg3 = I.scaled(I.CONFIGS["cfg2"], 17)
+    sched3 = ([3, 1, 0, 2, 3, 0], [1, 1, 2, 1, 2, 2])
+    check_parity(cfg3, 3, orc, sched=sched3)
+
+
+def test_ragged_dims_and_fewer_levels(orc):
+    """non-square / non-cubic grids, rows that are not a multiple of the 128-B pitch, levels < max."""
+    import dataclasses
+    base = I.CONFIGS["cfg1"]
+    cfg = dataclasses.replace(base, name="cfg1@ragged", dims=(49, 81), levels=4)
+    check_parity(cfg, 4, orc)
+    base3 = I.CONFIGS["cfg5"]
+    cfg3 = dataclasses.replace(base3, name="cfg5@ragged", dims=(17, 41, 25), levels=3)
+    check_parity(cfg3, 4, orc)
+    cfg4 = dataclasses.replace(I.CONFIGS["cfg4"], name="cfg4@ragged", dims=(9, 13, 37), levels=2)
+    check_parity(cfg4, 4, orc)
+
+
+def test_single_level_and_smallest_grid(orc):
+    import dataclasses
+    cfg = dataclasses.replace(I.CONFIGS["cfg1"], name="cfg1@1lvl", dims=(9, 9), levels=1)
+    check_parity(cfg, 3, orc)
+    cfg = dataclasses.replace(I.CONFIGS["cfg2"], name="cfg2@3", dims=(3, 3, 3), levels=1)
+    check_parity(cfg, 2, orc)
+    cfg = dataclasses.replace(I.CONFIGS["cfg2"], name="cfg2@5", dims=(5, 5, 5), levels=2)
+    check_parity(cfg, 3, orc)
+
+
+def test_graph_and_stream_launch_agree(orc):
+    cfg = I.scaled(I.CONFIGS["cfg2"], 33)
+    inp = I.make_inputs(cfg)
+    a, na, _ = run_gpu(cfg, inp, 3, use_graph=1)
+    b, nb, _ = run_gpu(cfg, inp, 3, use_graph=0)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert np.array_equal(na, nb)
+
+
+def test_device_arrays_and_zero_residual_fixed_point(orc):
+    """device-pointer in/out path; f = 0, u0 = 0 stays exactly 0 (pin P1's trivial half on the GPU)."""
+    torch = _torch()
+    from paper_1108_2045_b200 import homg
+    cfg = I.scaled(I.CONFIGS["cfg4"], 33)
+    inp = I.make_inputs(cfg)
+    s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype)
+    fd = torch.from_numpy(inp["f"]).cuda()
+    s.set_rhs(fd)
+    s.cycle(3)
+    out = torch.empty(cfg.dims, dtype=torch.float32, device="cuda")
+    s.get_solution(out)
+    host = np.empty(cfg.dims, dtype=np.float32)
+    s.get_solution(host)
+    assert np.array_equal(out.cpu().numpy(), host)
+    s.set_rhs(torch.zeros_like(fd))
+    s.set_initial_guess(torch.zeros_like(fd))
+    s.cycle(2)
+    s.get_solution(host)
+    assert not host.any()
+    assert s.residual_norm()[0] == 0.0
+    s.destroy()
+
+
+def test_error_paths():
+    _torch()
+    from paper_1108_2045_b200 import homg
+    with pytest.raises(homg.HomgError):
+        homg.Solver((130, 129), 7, "poisson5", "f64")
+    with pytest.raises(homg.HomgError):
+        homg.Solver((129, 129), 7, "poisson7", "f64")
+    s = homg.Solver((17, 17), 3, "poisson5", "f64")
+    with pytest.raises(homg.HomgError) as ei:
+        s.cycle(1)
+    assert ei.value.status == homg.HOMG_ESTATE
+    s.destroy()
+    s = homg.Solver((9, 9, 9), 2, "diffusion7", "f64")
+    s.set_rhs(np.ones((9, 9, 9)))
+    with pytest.raises(homg.HomgError):
+        s.cycle(1)
+    s.destroy()
