@@ -140,6 +140,29 @@ HOMG_API int homg_get_schedule(const homg_solver* s, int* levels_out, int* iters
 HOMG_API int homg_launches_per_cycle(const homg_solver* s);
 HOMG_API double homg_bytes_per_cycle(const homg_solver* s, int level0_only);
 
+/* Measurement aid (bench.py): runs n cycles with plain stream launches and a CUDA event after every
+ * launch, and accumulates per kernel class the elapsed milliseconds and the launch count into
+ * ms_by_tag / launches_by_tag, and the ALGORITHMIC bytes those launches must move (DESIGN.md
+ * "Roofline": array passes x nodes x scalar size) into bytes_by_tag (host arrays, cap >= HOMG_TAG_COUNT).  The cycles are real:
+ * u advances and n history entries are appended.  Synchronises the stream. */
+enum {
+    HOMG_TAG_RESIDUAL0 = 0, /* level-0 residual (+norm partials, + first restriction when fused) */
+    HOMG_TAG_NORM_FINISH,   /* fixed-order sum of the partials                                    */
+    HOMG_TAG_RESTRICT,      /* full weighting g_m = P g_{m-1}                                     */
+    HOMG_TAG_RELAX0,        /* level-0 Jacobi sweeps (incl. fused interpolate+correct, u += e)    */
+    HOMG_TAG_RELAX,         /* Jacobi sweeps on levels >= 1                                       */
+    HOMG_TAG_DELIVER0,      /* interpolate+correct onto level 0 when not fused into the sweep     */
+    HOMG_TAG_DELIVER,       /* interpolate+correct onto levels >= 1                               */
+    HOMG_TAG_INJECT,
+    HOMG_TAG_D0,            /* carried variation                                                  */
+    HOMG_TAG_COARSE,        /* the persistent coarse-level launch                                 */
+    HOMG_TAG_OTHER,
+    HOMG_TAG_COUNT
+};
+HOMG_API homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* launches_by_tag,
+                                         double* bytes_by_tag, int cap);
+HOMG_API const char* homg_tag_name(int tag);
+
 HOMG_API void homg_destroy(homg_solver* s);
 
 /* Text of the last error on this solver ("" if none).  s may be NULL: returns the text

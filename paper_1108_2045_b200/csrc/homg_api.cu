@@ -9,6 +9,8 @@
 
 using namespace homg;
 
+static_assert(int(TAG_COUNT) == int(HOMG_TAG_COUNT), "tag tables out of sync");
+
 namespace {
 
 thread_local std::string g_create_err;
@@ -233,6 +235,23 @@ homg_status homg_get_solution(homg_solver* s, void* dst, int on_device) {
         CU(s, cudaStreamSynchronize(s->stream));
     }
     return HOMG_OK;
+}
+
+homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* launches_by_tag,
+                                double* bytes_by_tag, int cap) {
+    if (!s) return HOMG_EINVAL;
+    if (!ms_by_tag || !launches_by_tag || !bytes_by_tag || cap < HOMG_TAG_COUNT) return set_err(s, HOMG_EINVAL, "profile arrays too small");
+    if (!s->have_rhs || (s->var && !s->have_coef)) return set_err(s, HOMG_ESTATE, "profile before set_rhs / set_coefficient");
+    for (int i = 0; i < cap; ++i) { ms_by_tag[i] = 0.0; launches_by_tag[i] = 0; bytes_by_tag[i] = 0.0; }
+    for (int c = 0; c < n; ++c) CU(s, exec_cycle_profiled(s, s->stream, ms_by_tag, launches_by_tag, bytes_by_tag));
+    s->cycles_issued += n;
+    return HOMG_OK;
+}
+
+const char* homg_tag_name(int tag) {
+    static const char* names[HOMG_TAG_COUNT] = {"residual_l0", "norm_finish", "restrict", "relax_l0", "relax_coarse",
+                                                "deliver_l0", "deliver", "inject", "d0", "coarse_persistent", "other"};
+    return (tag >= 0 && tag < HOMG_TAG_COUNT) ? names[tag] : "";
 }
 
 int homg_get_schedule(const homg_solver* s, int* lv, int* it, int cap) {

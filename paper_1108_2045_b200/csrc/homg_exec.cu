@@ -15,14 +15,27 @@ struct Rec {                 // bookkeeping while recording
     cudaError_t err = cudaSuccess;
     int launches = 0;
     double bytes_all = 0, bytes_l0 = 0;
-    void check() {
+    std::vector<cudaEvent_t>* ev = nullptr;   // profile mode: one event after every launch
+    std::vector<int>* ev_tag = nullptr;
+    int last_tag = TAG_OTHER;
+    double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class
+    void check(int tag) {
+        last_tag = tag;
         cudaError_t e = cudaPeekAtLastError();
         if (err == cudaSuccess && e != cudaSuccess) err = e;
         ++launches;
+        if (ev) {
+            cudaEvent_t x;
+            cudaEventCreate(&x);
+            cudaEventRecord(x, st);
+            ev->push_back(x);
+            ev_tag->push_back(tag);
+        }
     }
     void acct(int level, double arrays) {     // `arrays` passes over one level-`level` array
         double b = arrays * double(s->L[level].n_nodes) * double(s->dtype);
         bytes_all += b;
+        bytes_tag[last_tag] += b;
         if (level == 0) bytes_l0 += b;
     }
 };
@@ -51,12 +64,12 @@ void rec_norm(Rec& R, bool write_r, bool to_history) {
     dim3 g = grd(L0.g);
     k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
                                                    (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
-    R.check();
+    R.check(TAG_RESIDUAL0);
     R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
     int n = int(g.x * g.y * g.z);
     k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
                                         to_history ? 1 : 0, to_history ? nullptr : s->scalar);
-    R.check();
+    R.check(TAG_NORM_FINISH);
 }
 
 template <class T, int ND, bool VAR>
@@ -73,7 +86,7 @@ void rec_cycle(Rec& R) {
     // S2: nested restriction g_m = P g_{m-1}
     for (int m = 1; m <= M; ++m) {
         k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
-        R.check();
+        R.check(TAG_RESTRICT);
         R.acct(m - 1, 1.0); R.acct(m, 1.0);
     }
     // S3: MFMG visits
@@ -85,7 +98,7 @@ void rec_cycle(Rec& R) {
         bool have_d0 = false;
         if (cur < 0) {
             cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
-            R.check();
+            R.check(TAG_OTHER);
             Lt.touched = true;
         } else {
             if (t < cur) {
@@ -99,7 +112,7 @@ void rec_cycle(Rec& R) {
                     if (af_mode == 2 && !ac) af_mode = 0;          // 0 + 0: a stays "known zero"
                     k_deliver<T, ND><<<grd(Lf.g), blk(), 0, R.st>>>(Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
                                                                      rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
-                    R.check();
+                    R.check(m - 1 == 0 ? TAG_DELIVER0 : TAG_DELIVER);
                     R.acct(m, ac ? 2.0 : 1.0);
                     R.acct(m - 1, (ef_assign ? 1.0 : 2.0) + (af_mode == 1 ? 2.0 : af_mode == 2 ? 1.0 : 0.0));
                     Lf.touched = true;
@@ -111,7 +124,7 @@ void rec_cycle(Rec& R) {
                 for (int m = cur + 1; m <= t; ++m) {
                     k_inject<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
                                                                       rotp<T>(L[m], L[m].e));
-                    R.check();
+                    R.check(TAG_INJECT);
                     R.acct(m, 2.0);
                     L[m].touched = true;
                 }
@@ -123,7 +136,7 @@ void rec_cycle(Rec& R) {
                 const T* Y = rotp<T>(Lv, Lv.vkm1);
                 if (t >= cur) {
                     k_d0_up<T, ND><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
-                    R.check();
+                    R.check(TAG_D0);
                     R.acct(t, 3.0);
                 } else {
                     const T* A = dp_is_d0[cur] ? (const T*)Lv.d0 : rotp<T>(Lv, Lv.vkm1);
@@ -133,7 +146,7 @@ void rec_cycle(Rec& R) {
                         T* out = last ? (T*)Lt.d0 : (T*)L[m - 1].tmp;
                         k_d0_down<T, ND><<<grd(L[m - 1].g), blk(), 0, R.st>>>(L[m - 1].g, L[m].g, A, B, out,
                                                                                last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
-                        R.check();
+                        R.check(TAG_D0);
                         R.acct(m, B ? 2.0 : 1.0); R.acct(m - 1, 1.0);
                         A = out; B = nullptr;
                     }
@@ -143,7 +156,7 @@ void rec_cycle(Rec& R) {
         }
         if (t >= 1 && !have_d0 && eta == 1) {        // first visit with eta = 1: its dp is d0 = 0
             cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st);
-            R.check();
+            R.check(TAG_OTHER);
             have_d0 = true;
         }
         // S3d eta damped-Jacobi sweeps; S3e bookkeeping fused into the last one; S4 u += e fused
@@ -162,7 +175,7 @@ void rec_cycle(Rec& R) {
                 Lt.g, cf, rotp<T>(Lt, in), (const T*)Lt.gsrc, (const T*)Lt.k, rotp<T>(Lt, out),
                 book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0),
                 addu ? (T*)s->u : nullptr);
-            R.check();
+            R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
             R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
                           (addu ? 2.0 : 0.0));
             prev2 = prev_in; prev_in = in; in = out;
@@ -180,7 +193,7 @@ void rec_sample(Rec& R) {
     for (int m = 1; m < s->levels; ++m) {
         k_sample_coef<T, ND><<<grd(s->L[m].g), blk(), 0, R.st>>>(s->L[m].g, s->L[m - 1].g, (const T*)s->L[m - 1].k,
                                                                    (T*)s->L[m].k);
-        R.check();
+        R.check(TAG_OTHER);
     }
 }
 
@@ -188,14 +201,14 @@ template <class T, int ND>
 void rec_pack(Rec& R, const void* dense, void* padded, int zero_boundary) {
     const LevelGeom& g = R.s->L[0].g;
     k_pack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)dense, (T*)padded, zero_boundary);
-    R.check();
+    R.check(TAG_OTHER);
 }
 
 template <class T, int ND>
 void rec_unpack(Rec& R, const void* padded, void* dense) {
     const LevelGeom& g = R.s->L[0].g;
     k_unpack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)padded, (T*)dense);
-    R.check();
+    R.check(TAG_OTHER);
 }
 
 // dispatch on (dtype, ndim, var)
@@ -229,6 +242,32 @@ cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     s->launches_per_cycle = R.launches;
     s->bytes_cycle_all = R.bytes_all;
     s->bytes_cycle_l0 = R.bytes_l0;
+    return R.err;
+}
+
+cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_tag, int* launches_by_tag,
+                                double* bytes_by_tag) {
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> tag;
+    cudaEvent_t e0;
+    cudaEventCreate(&e0);
+    cudaEventRecord(e0, st);
+    Rec R{s, st};
+    R.ev = &ev; R.ev_tag = &tag;
+    HOMG_DISPATCH(s, rec_cycle, R);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (R.err == cudaSuccess) R.err = e;
+    cudaEvent_t prev = e0;
+    for (size_t i = 0; i < ev.size(); ++i) {
+        float ms = 0.f;
+        if (R.err == cudaSuccess) cudaEventElapsedTime(&ms, prev, ev[i]);
+        ms_by_tag[tag[i]] += double(ms);
+        launches_by_tag[tag[i]] += 1;
+        prev = ev[i];
+    }
+    for (int t = 0; t < TAG_COUNT; ++t) bytes_by_tag[t] += R.bytes_tag[t];
+    cudaEventDestroy(e0);
+    for (auto x : ev) cudaEventDestroy(x);
     return R.err;
 }
 

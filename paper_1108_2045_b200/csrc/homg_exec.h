@@ -4,9 +4,19 @@
 
 namespace homg {
 
+// kernel classes reported by homg_profile_cycles (order = include/homg.h HOMG_TAG_*)
+enum {
+    TAG_RESIDUAL0 = 0, TAG_NORM_FINISH, TAG_RESTRICT, TAG_RELAX0, TAG_RELAX, TAG_DELIVER0, TAG_DELIVER,
+    TAG_INJECT, TAG_D0, TAG_COARSE, TAG_OTHER, TAG_COUNT
+};
+
 // Issues the launches of ONE outer cycle on `st` (which may be a capturing stream) and fills
 // s->launches_per_cycle / s->bytes_cycle_*.
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st);
+// One cycle with plain stream launches, an event after every launch; accumulates the elapsed ms and
+// launch counts per TAG_* (arrays of TAG_COUNT).  Synchronises the stream.
+cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_tag, int* launches_by_tag,
+                                double* bytes_by_tag);
 // ||f - A u||^2 of the current u -> *s->scalar (no history entry).
 cudaError_t exec_norm_only(homg_solver* s, cudaStream_t st);
 // k_m = k_{m-1} sampled at even nodes, m = 1..M.

@@ -70,7 +70,6 @@ __device__ __forceinline__ T node_jacobi(const T* __restrict__ v, const T* __res
                                          long long c, const LevelGeom& g, const Coef<T>& cf) {
     T Av, D;
     node_A<T, ND, VAR>(v, k, c, g, cf, Av, D);
-    if (!VAR) return v[c] + cf.w_over_D * (gval - Av);
     return v[c] + cf.w * (gval - Av) / D;
 }
 
