@@ -86,6 +86,10 @@ typedef struct {
     int use_graph;    /* 1 (default when < 0): replay one CUDA graph per cycle; 0: plain
                          stream launches (debugging, profiling)                          */
     int history_cap;  /* capacity of the device-side norm history; <= 0: 4096            */
+    int tiled_min_nodes; /* levels with >= this many nodes run the TMA-tiled kernels; 0: library
+                            default; < 0: never (generic kernels only)                     */
+    int march_chunk;  /* planes per CTA along the marching axis of the tiled kernels; <= 0:
+                         chosen from the SM count                  */
     void* cuda_stream; /* cudaStream_t; NULL = legacy default stream                     */
 } homg_options;
 

@@ -2,6 +2,7 @@
 // graph capture and replay.  No arithmetic of the method happens on the host.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -98,6 +99,10 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     s->max_iters = o.max_iters > 0 ? o.max_iters : 4;
     s->coarse_threshold = o.coarse_threshold_nodes;
     s->use_graph = o.use_graph != 0;
+    s->tiled_min_nodes = o.tiled_min_nodes > 0 ? o.tiled_min_nodes : (o.tiled_min_nodes < 0 ? -1 : kTiledMinNodesDefault);
+    if (const char* ev = std::getenv("HOMG_TILED_MIN_NODES")) s->tiled_min_nodes = std::atoll(ev);
+    s->march_chunk = o.march_chunk > 0 ? o.march_chunk : 0;
+    if (const char* ev = std::getenv("HOMG_MARCH_CHUNK")) s->march_chunk = std::atoi(ev);
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);
     s->hist_cap = hist_cap;
     if (build_schedule(o.schedule, levels, s->max_iters, o.sched_levels, o.sched_iters, o.sched_len, s->sched_lv,
@@ -133,6 +138,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (size_t(p - s->ws_base) > ws_bytes) { delete s; return set_err(nullptr, HOMG_ENOMEM, "internal: layout exceeds plan"); }
 
     cudaError_t e = cudaMemsetAsync(ws, 0, size_t(p - s->ws_base), s->stream);
+    if (e == cudaSuccess) e = exec_init(s);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking);
     if (e != cudaSuccess) {
         homg_status r = cuda_fail(nullptr, e, "homg_create");

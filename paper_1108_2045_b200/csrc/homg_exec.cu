@@ -3,7 +3,9 @@
 // by homg_api.cu).  Host logic only decides pointers and flags; every arithmetic step is a kernel.
 #include "homg_exec.h"
 
-#include "homg_kernels.cuh"
+#include <algorithm>
+
+#include "homg_fused.cuh"
 
 namespace homg {
 
@@ -56,6 +58,75 @@ Coef<T> make_coef(const homg_solver* s, int m) {
 
 template <class T>
 T* rotp(Level& L, int i) { return i < 0 ? nullptr : static_cast<T*>(L.rot[i]); }
+
+
+// ---- TMA tensor maps (encoded on the host by the driver's cuTensorMapEncodeTiled) ----------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// map over one level array: dims (nx, ny[, nz]), row pitch px, plane pitch pp; box (bx, by[, 1]).
+// Elements outside [0,nx) x [0,ny) x [0,nz) are delivered as 0 (the Dirichlet value / pad).
+template <class T, int ND>
+bool make_tmap(const homg_solver* s, CUtensorMap* tm, const void* base, const LevelGeom& g, int bx, int by) {
+    cuuint64_t gdim[3] = {cuuint64_t(g.nx), cuuint64_t(g.ny), cuuint64_t(g.nz)};
+    cuuint64_t gstr[2] = {cuuint64_t(g.px) * sizeof(T), cuuint64_t(g.pp) * sizeof(T)};
+    cuuint32_t box[3] = {cuuint32_t(bx), cuuint32_t(by), 1};
+    cuuint32_t est[3] = {1, 1, 1};
+    CUtensorMapDataType dt = sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+    CUresult r = reinterpret_cast<EncodeTiledFn>(s->encode_tiled)(
+        tm, dt, ND, const_cast<void*>(base), gdim, gstr, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+inline bool tiled(const homg_solver* s, int m) {
+    return s->encode_tiled && s->tiled_min_nodes > 0 && s->L[m].n_nodes >= s->tiled_min_nodes;
+}
+
+// planes per CTA along the marching axis: as few chunks as fill the machine about once
+template <class T, int ND>
+int march_chunk(const homg_solver* s, const LevelGeom& g, int* nchunks) {
+    using TL = Tile<T, ND>;
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const int interior = std::max(NM - 2, 1);
+    long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
+    int mc = s->march_chunk;
+    if (mc <= 0) {
+        long long slots = (long long)s->sm_count * 4;
+        long long nch = std::max<long long>(1, slots / std::max<long long>(tiles, 1));
+        mc = int((interior + nch - 1) / nch);
+        mc = std::max(mc, 8);
+    }
+    mc = std::min(mc, interior);
+    *nchunks = (interior + mc - 1) / mc;
+    return mc;
+}
+
+// one Jacobi sweep on level t (tiled or generic), with the optional epilogues of k_relax
+template <class T, int ND, bool VAR>
+void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, const T* d0, const T* v0, T* u) {
+    homg_solver* s = R.s;
+    Level& Lt = s->L[t];
+    Coef<T> cf = make_coef<T>(s, t);
+    if (tiled(s, t)) {
+        using TL = Tile<T, ND>;
+        CUtensorMap tmv, tmg, tmk;
+        bool ok = make_tmap<T, ND>(s, &tmv, vin, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1) &&
+                  make_tmap<T, ND>(s, &tmg, Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
+        if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, Lt.k, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1);
+        else tmk = tmv;
+        if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
+        int nch = 1;
+        int mc = march_chunk<T, ND>(s, Lt.g, &nch);
+        dim3 grid((Lt.g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (Lt.g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
+        k_relax_tma<T, ND, VAR><<<grid, 256, relax_smem_bytes<T, ND, VAR>(), R.st>>>(tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
+                                                                                      d0, v0, u, mc);
+    } else {
+        k_relax<T, ND, VAR><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, cf, vin, (const T*)Lt.gsrc, (const T*)Lt.k, vout, a,
+                                                            a_assign, d0, v0, u);
+    }
+}
 
 template <class T, int ND, bool VAR>
 void rec_norm(Rec& R, bool write_r, bool to_history) {
@@ -163,7 +234,6 @@ void rec_cycle(Rec& R) {
         // into the last sweep of the cycle.
         const int v0 = Lt.e;
         int in = v0, prev_in = -1, prev2 = -1;
-        Coef<T> cf = make_coef<T>(s, t);
         for (int it = 0; it < eta; ++it) {
             int out = -1;
             for (int b = 0; b < Lt.nrot; ++b)
@@ -171,10 +241,8 @@ void rec_cycle(Rec& R) {
             bool last = (it == eta - 1);
             bool book = last && t >= 1;
             bool addu = last && vi == nv - 1;
-            k_relax<T, ND, VAR><<<grd(Lt.g), blk(), 0, R.st>>>(
-                Lt.g, cf, rotp<T>(Lt, in), (const T*)Lt.gsrc, (const T*)Lt.k, rotp<T>(Lt, out),
-                book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0),
-                addu ? (T*)s->u : nullptr);
+            launch_relax<T, ND, VAR>(R, t, rotp<T>(Lt, in), rotp<T>(Lt, out), book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0,
+                                     have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
             R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
             R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
                           (addu ? 2.0 : 0.0));
@@ -234,7 +302,34 @@ void rec_unpack(Rec& R, const void* padded, void* dense) {
         }                                                                                    \
     } while (0)
 
+
+template <class T, int ND, bool VAR>
+cudaError_t set_attr() {
+    return cudaFuncSetAttribute(k_relax_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                relax_smem_bytes<T, ND, VAR>());
+}
+
 }  // namespace
+
+cudaError_t exec_init(homg_solver* s) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) return e != cudaSuccess ? e : cudaErrorNotSupported;
+    s->encode_tiled = fn;
+    if ((e = set_attr<float, 2, false>()) != cudaSuccess) return e;
+    if ((e = set_attr<float, 3, false>()) != cudaSuccess) return e;
+    if ((e = set_attr<float, 3, true>()) != cudaSuccess) return e;
+    if ((e = set_attr<double, 2, false>()) != cudaSuccess) return e;
+    if ((e = set_attr<double, 3, false>()) != cudaSuccess) return e;
+    if ((e = set_attr<double, 3, true>()) != cudaSuccess) return e;
+    return cudaSuccess;
+}
 
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     Rec R{s, st};

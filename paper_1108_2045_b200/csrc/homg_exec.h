@@ -10,6 +10,11 @@ enum {
     TAG_INJECT, TAG_D0, TAG_COARSE, TAG_OTHER, TAG_COUNT
 };
 
+constexpr long long kTiledMinNodesDefault = 200000;   // 65^3 and up, 449^2 and up
+
+// Device queries, the driver's tensor-map encoder, kernel attributes.  Called once by homg_create.
+cudaError_t exec_init(homg_solver* s);
+
 // Issues the launches of ONE outer cycle on `st` (which may be a capturing stream) and fills
 // s->launches_per_cycle / s->bytes_cycle_*.
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st);

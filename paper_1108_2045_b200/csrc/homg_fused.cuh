@@ -1,0 +1,211 @@
+// homg_fused.cuh — tiled sm_100a kernels for the LARGE levels of the HOMG cycle.
+//
+// Common scheme (north_star items 2-3): a CTA of 256 threads owns an x/y tile and marches along the
+// slowest axis (z in 3-D, y in 2-D).  Every plane of the tile (plus halo) is brought into a 4-stage
+// shared-memory ring by TMA (cp.async.bulk.tensor, completion on an mbarrier), three planes ahead of
+// the one being computed; out-of-range halo elements arrive as 0, which is the Dirichlet value.
+// Threads hold VEC = 16 B / sizeof(T) consecutive x nodes each (LDS.128 / STG.128) and keep the
+// previous / current / next plane of their own nodes in registers (register blocking along the
+// slowest axis), so shared memory is read only for the in-plane neighbours.
+//
+// The arithmetic is the expression tree of homg_kernels.cuh (R14) — results are bit-identical
+// to the generic kernels and to the oracle.
+#pragma once
+#include "homg_kernels.cuh"
+#include "homg_tma.cuh"
+
+namespace homg {
+
+template <class T>
+struct alignas(16) Pack {
+    T v[16 / sizeof(T)];
+};
+
+template <class T, int ND>
+struct Tile {
+    static constexpr int VEC = 16 / int(sizeof(T));
+    static constexpr int WY = ND == 3 ? 8 : 1;           // warps along y
+    static constexpr int WX = 8 / WY;                    // warps (segments) along x
+    static constexpr int SEG = 32 * VEC;                 // x nodes per warp
+    static constexpr int TX = WX * SEG, TY = WY;         // nodes per CTA and plane
+    static constexpr int VW = SEG + 2 * VEC;             // halo'd row width (one TMA box row)
+    static constexpr int VROWS = ND == 3 ? TY + 2 : WX;  // rows of the halo'd tile in shared memory
+    // 3-D: one box {VW, TY+2, 1}, rows contiguous.  2-D: WX boxes {VW, 1}, each 128-B aligned.
+    static constexpr int VRS = ND == 3 ? VW : ((VW * int(sizeof(T)) + 127) / 128 * 128) / int(sizeof(T));
+    static constexpr int VBOX_BYTES = VROWS * VW * int(sizeof(T));             // bytes TMA delivers
+    static constexpr int VTILE_BYTES = (VROWS * VRS * int(sizeof(T)) + 127) / 128 * 128;
+    static constexpr int GROWS = ND == 3 ? TY : WX;
+    static constexpr int GBOX_BYTES = GROWS * SEG * int(sizeof(T));            // = tile bytes (128-B multiple)
+    static constexpr int NST = 4;
+};
+
+template <class T, int ND, bool VAR>
+__host__ __device__ constexpr int relax_stage_bytes() {
+    return Tile<T, ND>::VTILE_BYTES * (VAR ? 2 : 1) + Tile<T, ND>::GBOX_BYTES;
+}
+template <class T, int ND, bool VAR>
+__host__ __device__ constexpr int relax_smem_bytes() {
+    return relax_stage_bytes<T, ND, VAR>() * Tile<T, ND>::NST + 128;
+}
+
+// S3d (+S3e, +S4): one damped-Jacobi sweep  vout = vin + w (g - A vin)/D  on a large level.
+//   tmv / tmk / tmg : tensor maps of vin, k (VAR) and g of this level
+//   a, a_assign, d0, v0, u : the optional epilogues of k_relax (same meaning)
+//   mchunk : interior planes per CTA along the marching axis
+// grid = (x tiles, y tiles, chunks) in 3-D, (x tiles, chunks) in 2-D.      (Eq.2-3)
+template <class T, int ND, bool VAR>
+__global__ void __launch_bounds__(256)
+k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUtensorMap tmg,
+            const __grid_constant__ CUtensorMap tmk, LevelGeom g, Coef<T> cf, T* __restrict__ vout,
+            T* __restrict__ a, int a_assign, const T* __restrict__ d0, const T* __restrict__ v0,
+            T* __restrict__ u, int mchunk) {
+    using TL = Tile<T, ND>;
+    constexpr int VEC = TL::VEC;
+    constexpr int STAGE = relax_stage_bytes<T, ND, VAR>();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wx = warp % TL::WX, wy = warp / TL::WX;
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const long long mstride = ND == 3 ? g.pp : (long long)g.px;
+    const int x0 = blockIdx.x * TL::TX;
+    const int y0 = ND == 3 ? blockIdx.y * TL::TY : 0;
+    const int chunk = ND == 3 ? blockIdx.z : blockIdx.y;
+    const int ms = 1 + chunk * mchunk;
+    const int me = min(ms + mchunk, NM - 1);
+    if (ms >= me) return;
+    const int count = me - ms + 2;                       // planes ms-1 .. me
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    __shared__ uint64_t bars[TL::NST];
+    auto vs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
+    auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES); };
+    auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES * (VAR ? 2 : 1)); };
+
+    if (tid == 0) {
+        for (int s = 0; s < TL::NST; ++s) mbar_init(&bars[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto issue = [&](int i) {                            // relative plane i = absolute ms-1+i
+        const int st = i & (TL::NST - 1), p = ms - 1 + i;
+        const bool wantg = i >= 1 && i <= count - 2;
+        mbar_arrive_expect_tx(&bars[st], TL::VBOX_BYTES * (VAR ? 2 : 1) + (wantg ? TL::GBOX_BYTES : 0));
+        if (ND == 3) {
+            tma_load_3d(vs(st), &tmv, &bars[st], x0 - VEC, y0 - 1, p);
+            if (VAR) tma_load_3d(ks(st), &tmk, &bars[st], x0 - VEC, y0 - 1, p);
+            if (wantg) tma_load_3d(gs(st), &tmg, &bars[st], x0, y0, p);
+        } else {
+            for (int w = 0; w < TL::WX; ++w) {
+                tma_load_2d(vs(st) + w * TL::VRS, &tmv, &bars[st], x0 + w * TL::SEG - VEC, p);
+                if (wantg) tma_load_2d(gs(st) + w * TL::SEG, &tmg, &bars[st], x0 + w * TL::SEG, p);
+            }
+        }
+    };
+
+    // this thread's nodes: x .. x+VEC-1 of row y; its row inside the halo'd tile
+    const int x = x0 + wx * TL::SEG + lane * VEC;
+    const int y = ND == 3 ? y0 + wy : 0;
+    const int vrow = ND == 3 ? wy + 1 : wx;
+    const int voff = vrow * TL::VRS + VEC + lane * VEC;  // centre pack inside a v / k tile
+    const int goff = (ND == 3 ? wy : wx) * TL::SEG + lane * VEC;
+    const bool row_ok = x < g.nx && (ND == 2 || y < g.ny);
+    const bool row_int = ND == 2 || (y > 0 && y < g.ny - 1);
+    bool xin[VEC];
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) xin[j] = row_int && (x + j > 0) && (x + j < g.nx - 1);
+
+    if (tid == 0)
+        for (int i = 0; i < TL::NST && i < count; ++i) issue(i);
+
+    Pack<T> prv, cur, nxt, kprv, kcur, knxt;
+    mbar_wait(&bars[0], 0);
+    prv = *reinterpret_cast<const Pack<T>*>(vs(0) + voff);
+    if (VAR) kprv = *reinterpret_cast<const Pack<T>*>(ks(0) + voff);
+    mbar_wait(&bars[1], 0);
+    cur = *reinterpret_cast<const Pack<T>*>(vs(1) + voff);
+    if (VAR) kcur = *reinterpret_cast<const Pack<T>*>(ks(1) + voff);
+    __syncthreads();
+    if (tid == 0 && TL::NST < count) issue(TL::NST);
+
+    long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
+    for (int i = 1; i <= count - 2; ++i, c += mstride) {
+        const int sn = (i + 1) & (TL::NST - 1), sc = i & (TL::NST - 1);
+        mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
+        nxt = *reinterpret_cast<const Pack<T>*>(vs(sn) + voff);
+        if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
+        const T* vt = vs(sc);
+        const T* kt = ks(sc);
+        Pack<T> dn, up, kdn, kup;
+        if (ND == 3) {
+            dn = *reinterpret_cast<const Pack<T>*>(vt + voff - TL::VRS);
+            up = *reinterpret_cast<const Pack<T>*>(vt + voff + TL::VRS);
+            if (VAR) {
+                kdn = *reinterpret_cast<const Pack<T>*>(kt + voff - TL::VRS);
+                kup = *reinterpret_cast<const Pack<T>*>(kt + voff + TL::VRS);
+            }
+        }
+        const T vl = vt[voff - 1], vr = vt[voff + VEC];
+        T kl = T(0), kr = T(0);
+        if (VAR) { kl = kt[voff - 1]; kr = kt[voff + VEC]; }
+        const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs(sc) + goff);
+        Pack<T> out;
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) {
+            const T vc = cur.v[j];
+            const T xm = j == 0 ? vl : cur.v[j - 1 < 0 ? 0 : j - 1];
+            const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+            T Av, D;
+            if (!VAR) {
+                T s = T(0);
+                s += prv.v[j] + nxt.v[j];
+                if (ND == 3) s += dn.v[j] + up.v[j];
+                s += xm + xp;
+                Av = (cf.twod * vc - s) * cf.ih2;
+                D = cf.twod * cf.ih2;
+            } else {
+                const T kc = kcur.v[j];
+                const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
+                const T kxp = j == VEC - 1 ? kr : kcur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+                T acc = T(0), ds = T(0), kf;
+                kf = kface(kc, kprv.v[j]); acc += kf * (vc - prv.v[j]); ds += kf;
+                kf = kface(kc, knxt.v[j]); acc += kf * (vc - nxt.v[j]); ds += kf;
+                if (ND == 3) {
+                    kf = kface(kc, kdn.v[j]); acc += kf * (vc - dn.v[j]); ds += kf;
+                    kf = kface(kc, kup.v[j]); acc += kf * (vc - up.v[j]); ds += kf;
+                }
+                kf = kface(kc, kxm); acc += kf * (vc - xm); ds += kf;
+                kf = kface(kc, kxp); acc += kf * (vc - xp); ds += kf;
+                Av = acc * cf.ih2;
+                D = ds * cf.ih2;
+            }
+            out.v[j] = xin[j] ? vc + cf.w * (gv.v[j] - Av) / D : T(0);
+        }
+        if (row_ok) {
+            *reinterpret_cast<Pack<T>*>(vout + c) = out;
+            if (a) {
+                Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(v0 + c), aa;
+                if (d0) dd = *reinterpret_cast<const Pack<T>*>(d0 + c);
+                if (!a_assign) aa = *reinterpret_cast<const Pack<T>*>(a + c);
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) {
+                    const T Dq = ((d0 ? dd.v[j] : T(0)) + cur.v[j]) - vv.v[j];
+                    aa.v[j] = a_assign ? Dq : aa.v[j] + Dq;
+                }
+                *reinterpret_cast<Pack<T>*>(a + c) = aa;
+            }
+            if (u) {
+                Pack<T> uu = *reinterpret_cast<const Pack<T>*>(u + c);
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) uu.v[j] += out.v[j];
+                *reinterpret_cast<Pack<T>*>(u + c) = uu;
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
+        prv = cur; cur = nxt;
+        if (VAR) { kprv = kcur; kcur = knxt; }
+    }
+}
+
+}  // namespace homg

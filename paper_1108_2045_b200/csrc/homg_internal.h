@@ -63,6 +63,10 @@ struct homg_solver {
     int max_iters = 4;
     int coarse_threshold = 0;
     bool use_graph = true;
+    long long tiled_min_nodes = 0;   // levels with >= this many nodes use the TMA-tiled kernels
+    int march_chunk = 0;             // 0: automatic
+    int sm_count = 148;
+    void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create
     std::vector<int> sched_lv, sched_it;
     std::vector<homg::Level> L;
     // level-0 extras

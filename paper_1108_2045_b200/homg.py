@@ -29,6 +29,7 @@ class HomgOptions(C.Structure):
         ("omega", C.c_double), ("h", C.c_double), ("max_iters", C.c_int), ("schedule", C.c_int),
         ("sched_levels", C.POINTER(C.c_int)), ("sched_iters", C.POINTER(C.c_int)), ("sched_len", C.c_int),
         ("coarse_threshold_nodes", C.c_int), ("use_graph", C.c_int), ("history_cap", C.c_int),
+        ("tiled_min_nodes", C.c_int), ("march_chunk", C.c_int),
         ("cuda_stream", C.c_void_p),
     ]
 
@@ -95,7 +96,8 @@ class Solver:
     """homg_create ... homg_destroy.  The workspace is a torch uint8 CUDA tensor owned by this object."""
 
     def __init__(self, dims, levels, stencil, dtype, omega=0.0, h=0.0, max_iters=0, schedule=HOMG_SCHED_C,
-                 sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, device="cuda:0", stream=None):
+                 sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, tiled_min_nodes=0,
+                 march_chunk=0, device="cuda:0", stream=None):
         import torch
         self._torch = torch
         self.dims = tuple(int(x) for x in dims)
@@ -110,6 +112,7 @@ class Solver:
         L.homg_default_options(C.byref(o))
         o.omega, o.h, o.max_iters, o.schedule = float(omega), float(h), int(max_iters), int(schedule)
         o.coarse_threshold_nodes, o.use_graph, o.history_cap = int(coarse_threshold_nodes), int(use_graph), int(history_cap)
+        o.tiled_min_nodes, o.march_chunk = int(tiled_min_nodes), int(march_chunk)
         self._keep = None
         if sched is not None:
             lv, it = sched

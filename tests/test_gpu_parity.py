@@ -199,3 +199,22 @@ def test_error_paths():
     with pytest.raises(homg.HomgError):
         s.cycle(1)
     s.destroy()
+
+
+@pytest.mark.parametrize("name,n,chunk", [("cfg2", 33, 0), ("cfg2", 65, 5), ("cfg4", 65, 0), ("cfg4", 129, 16),
+                                          ("cfg5", 33, 3), ("cfg5", 65, 0), ("cfg3", 257, 7), ("cfg3", 1025, 0),
+                                          ("cfg1", 129, 0)])
+def test_tiled_tma_kernels_every_level(orc, name, n, chunk):
+    """tiled_min_nodes=1 forces the TMA-tiled kernels on EVERY level (down to 3^d), with ragged
+    tiles, several chunks along the marching axis and chunk tails."""
+    ncyc = 2 if n >= 129 and name != "cfg1" and name != "cfg3" else 3
+    check_parity(I.scaled(I.CONFIGS[name], n), ncyc, orc, tiled_min_nodes=1, march_chunk=chunk)
+
+
+def test_tiled_matches_generic_bitwise(orc):
+    cfg = I.scaled(I.CONFIGS["cfg4"], 65)
+    inp = I.make_inputs(cfg)
+    a, na, _ = run_gpu(cfg, inp, 3, tiled_min_nodes=1)
+    b, nb, _ = run_gpu(cfg, inp, 3, tiled_min_nodes=-1)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
