@@ -128,19 +128,54 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
     }
 }
 
+// S1 (+S5, + first step of S2 when `restrict1`): r = f - A u, ||r||^2 -> history / scalar, g_1 = P r.
+// Returns true when g_1 was written by the fused kernel.
 template <class T, int ND, bool VAR>
-void rec_norm(Rec& R, bool write_r, bool to_history) {
+bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
     homg_solver* s = R.s;
     Level& L0 = s->L[0];
-    dim3 g = grd(L0.g);
-    k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
-                                                   (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
-    R.check(TAG_RESIDUAL0);
-    R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
-    int n = int(g.x * g.y * g.z);
+    int n = 0;
+    bool fused_restrict = false;
+    if (tiled(s, 0)) {
+        using TL = ResTile<T, ND>;
+        CUtensorMap tmu, tmf, tmk;
+        bool ok = make_tmap<T, ND>(s, &tmu, s->u, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1) &&
+                  make_tmap<T, ND>(s, &tmf, s->f, L0.g, TL::SEG, ND == 3 ? TL::TY + 1 : 1);
+        if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, L0.k, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1);
+        else tmk = tmu;
+        if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return false; }
+        fused_restrict = restrict1 && write_r && s->levels >= 2;
+        const LevelGeom& g = L0.g;
+        const int NM = ND == 3 ? g.nz : g.ny;
+        const int interior = std::max(NM - 2, 1);
+        long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
+        int mc = s->march_chunk;
+        if (mc <= 0) {
+            long long nch = std::max<long long>(1, (long long)s->sm_count * 3 / std::max<long long>(tiles, 1));
+            mc = std::max(int((interior + nch - 1) / nch), 8);
+        }
+        mc = (mc + 1) & ~1;                                        // even: chunks start on odd planes
+        int nch = (interior + mc - 1) / mc;
+        dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
+        n = int(grid.x * grid.y * grid.z);
+        k_res_tma<T, ND, VAR><<<grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), R.st>>>(
+            tmu, tmf, tmk, g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
+            fused_restrict ? (T*)s->L[1].gsrc : nullptr, s->partial, mc);
+        R.check(TAG_RESIDUAL0);
+        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
+        if (fused_restrict) R.acct(1, 1.0);
+    } else {
+        dim3 g = grd(L0.g);
+        k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
+                                                       (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
+        R.check(TAG_RESIDUAL0);
+        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
+        n = int(g.x * g.y * g.z);
+    }
     k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
                                         to_history ? 1 : 0, to_history ? nullptr : s->scalar);
     R.check(TAG_NORM_FINISH);
+    return fused_restrict;
 }
 
 template <class T, int ND, bool VAR>
@@ -153,9 +188,9 @@ void rec_cycle(Rec& R) {
     std::vector<char> dp_is_d0(s->levels, 0);    // eta == 1 visit: its dp is its own d0
 
     // S1: r = f - A u, ||r||^2 -> history
-    rec_norm<T, ND, VAR>(R, true, true);
+    const bool have_g1 = rec_norm<T, ND, VAR>(R, true, true, true);
     // S2: nested restriction g_m = P g_{m-1}
-    for (int m = 1; m <= M; ++m) {
+    for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
         k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
         R.check(TAG_RESTRICT);
         R.acct(m - 1, 1.0); R.acct(m, 1.0);
@@ -305,8 +340,11 @@ void rec_unpack(Rec& R, const void* padded, void* dense) {
 
 template <class T, int ND, bool VAR>
 cudaError_t set_attr() {
-    return cudaFuncSetAttribute(k_relax_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                relax_smem_bytes<T, ND, VAR>());
+    cudaError_t e = cudaFuncSetAttribute(k_relax_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         relax_smem_bytes<T, ND, VAR>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_res_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                res_smem_bytes<T, ND, VAR>());
 }
 
 }  // namespace
@@ -368,7 +406,7 @@ cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_t
 
 cudaError_t exec_norm_only(homg_solver* s, cudaStream_t st) {
     Rec R{s, st};
-    HOMG_DISPATCH(s, rec_norm, R, false, false);
+    HOMG_DISPATCH(s, rec_norm, R, false, false, false);
     return R.err;
 }
 

@@ -208,4 +208,221 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// K_res: fused residual + ||r||^2 partial + first full-weighting restriction (S1 + S2 first step + S5).
+//
+// The CTA computes r = f - A u on an r-tile that is one node wider than what it owns, on the low
+// side of every axis (full weighting of the coarse nodes of a tile needs r at 2I-1): 3-D: 9 warps,
+// warp R = fine row y0-1+R (row 0 is the recomputed halo row, rows 1..8 are owned); in every row
+// lane 0 holds the recomputed halo pack [xs-VEC, xs), lanes 1..31 the owned packs, so a tile owns
+// 31*VEC x 8 nodes per plane and every thread runs the same code.  2-D: 8 warps = 8 x-segments of
+// one row, each with its private halo pack.  The last four r planes stay in shared memory; after
+// an odd plane z = 2Z+1 the CTA writes the coarse plane Z (27 / 9 terms in the oracle's order).
+// A chunk [ms, me) of the marching axis (ms odd, even length) recomputes plane `me` for the same
+// reason.  r may be null (norm only); gc may be null (no restriction).
+//
+template <class T, int ND>
+struct ResTile {
+    static constexpr int VEC = 16 / int(sizeof(T));
+    static constexpr int NW = ND == 3 ? 9 : 8;           // warps
+    static constexpr int WX = ND == 3 ? 1 : 8;           // x segments
+    static constexpr int SEG = 32 * VEC;                 // r nodes per warp row (halo pack + owned)
+    static constexpr int OWN = 31 * VEC;                 // owned x nodes per segment
+    static constexpr int TX = WX * OWN, TY = ND == 3 ? 8 : 1;
+    static constexpr int UW = SEG + 2 * VEC;
+    static constexpr int UROWS = ND == 3 ? TY + 3 : WX;
+    static constexpr int URS = ND == 3 ? UW : ((UW * int(sizeof(T)) + 127) / 128 * 128) / int(sizeof(T));
+    static constexpr int UBOX_BYTES = UROWS * UW * int(sizeof(T));
+    static constexpr int UTILE_BYTES = (UROWS * URS * int(sizeof(T)) + 127) / 128 * 128;
+    static constexpr int FROWS = ND == 3 ? TY + 1 : WX;
+    static constexpr int FBOX_BYTES = FROWS * SEG * int(sizeof(T));
+    static constexpr int RPLANE = FROWS * SEG;           // elements of one r plane in shared memory
+    static constexpr int NST = 4, NR = 4;
+};
+template <class T, int ND, bool VAR>
+__host__ __device__ constexpr int res_stage_bytes() {
+    return ResTile<T, ND>::UTILE_BYTES * (VAR ? 2 : 1) + ResTile<T, ND>::FBOX_BYTES;
+}
+template <class T, int ND, bool VAR>
+__host__ __device__ constexpr int res_smem_bytes() {
+    return res_stage_bytes<T, ND, VAR>() * ResTile<T, ND>::NST +
+           ResTile<T, ND>::NR * ResTile<T, ND>::RPLANE * int(sizeof(T)) + 128;
+}
+
+template <class T, int ND, bool VAR>
+__global__ void __launch_bounds__(ResTile<T, ND>::NW * 32)
+k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUtensorMap tmf,
+          const __grid_constant__ CUtensorMap tmk, LevelGeom g, LevelGeom gcg, Coef<T> cf, T* __restrict__ r,
+          T* __restrict__ gc, double* __restrict__ partial, int mchunk) {
+    using TL = ResTile<T, ND>;
+    constexpr int VEC = TL::VEC;
+    constexpr int STAGE = res_stage_bytes<T, ND, VAR>();
+    const int tid = threadIdx.x, lane = tid & 31, R = tid >> 5;
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const long long mstride = ND == 3 ? g.pp : (long long)g.px;
+    const int x0 = blockIdx.x * TL::TX;
+    const int y0 = ND == 3 ? blockIdx.y * TL::TY : 0;
+    const int chunk = ND == 3 ? blockIdx.z : blockIdx.y;
+    const int ms = 1 + chunk * mchunk;
+    const int me = min(ms + mchunk, NM - 1);
+    const int nblk = gridDim.x * gridDim.y * gridDim.z;
+    const int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    (void)nblk;
+    if (ms >= me) { if (tid == 0) partial[bid] = 0.0; return; }
+    const int mlast = (gc != nullptr && me <= NM - 2) ? me : me - 1;   // last plane computed
+    const int count = mlast - ms + 3;                                  // u planes ms-1 .. mlast+1
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    __shared__ uint64_t bars[TL::NST];
+    auto us = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
+    auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES); };
+    auto fs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES * (VAR ? 2 : 1)); };
+    T* rring = reinterpret_cast<T*>(smem + TL::NST * STAGE);
+
+    if (tid == 0) {
+        for (int s = 0; s < TL::NST; ++s) mbar_init(&bars[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto issue = [&](int i) {
+        const int st = i & (TL::NST - 1), p = ms - 1 + i;
+        const bool wantf = i >= 1 && i <= count - 2;
+        mbar_arrive_expect_tx(&bars[st], TL::UBOX_BYTES * (VAR ? 2 : 1) + (wantf ? TL::FBOX_BYTES : 0));
+        if (ND == 3) {
+            tma_load_3d(us(st), &tmu, &bars[st], x0 - 2 * VEC, y0 - 2, p);
+            if (VAR) tma_load_3d(ks(st), &tmk, &bars[st], x0 - 2 * VEC, y0 - 2, p);
+            if (wantf) tma_load_3d(fs(st), &tmf, &bars[st], x0 - VEC, y0 - 1, p);
+        } else {
+            for (int w = 0; w < TL::WX; ++w) {
+                tma_load_2d(us(st) + w * TL::URS, &tmu, &bars[st], x0 + w * TL::OWN - 2 * VEC, p);
+                if (wantf) tma_load_2d(fs(st) + w * TL::SEG, &tmf, &bars[st], x0 + w * TL::OWN - VEC, p);
+            }
+        }
+    };
+
+    const int xs = ND == 3 ? x0 : x0 + R * TL::OWN;      // first owned x of this warp's segment
+    const int x = xs - VEC + lane * VEC;
+    const int y = ND == 3 ? y0 - 1 + R : 0;
+    const int urow = ND == 3 ? R + 1 : R;
+    const int voff = urow * TL::URS + VEC + lane * VEC;
+    const int foff = R * TL::SEG + lane * VEC;
+    const bool row_int = ND == 2 || (y > 0 && y < g.ny - 1);
+    const bool owned = lane >= 1 && x < g.nx && (ND == 2 || (R >= 1 && y < g.ny));
+    bool xin[VEC];
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) xin[j] = row_int && (x + j > 0) && (x + j < g.nx - 1);
+
+    if (tid == 0)
+        for (int i = 0; i < TL::NST && i < count; ++i) issue(i);
+
+    Pack<T> prv, cur, nxt, kprv, kcur, knxt;
+    mbar_wait(&bars[0], 0);
+    prv = *reinterpret_cast<const Pack<T>*>(us(0) + voff);
+    if (VAR) kprv = *reinterpret_cast<const Pack<T>*>(ks(0) + voff);
+    mbar_wait(&bars[1], 0);
+    cur = *reinterpret_cast<const Pack<T>*>(us(1) + voff);
+    if (VAR) kcur = *reinterpret_cast<const Pack<T>*>(ks(1) + voff);
+    __syncthreads();
+    if (tid == 0 && TL::NST < count) issue(TL::NST);
+
+    double sq = 0.0;
+    long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
+    for (int i = 1; i <= count - 2; ++i, c += mstride) {
+        const int z = ms - 1 + i;
+        const int sn = (i + 1) & (TL::NST - 1), sc = i & (TL::NST - 1);
+        mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
+        nxt = *reinterpret_cast<const Pack<T>*>(us(sn) + voff);
+        if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
+        const T* vt = us(sc);
+        const T* kt = ks(sc);
+        Pack<T> dn, up, kdn, kup;
+        if (ND == 3) {
+            dn = *reinterpret_cast<const Pack<T>*>(vt + voff - TL::URS);
+            up = *reinterpret_cast<const Pack<T>*>(vt + voff + TL::URS);
+            if (VAR) {
+                kdn = *reinterpret_cast<const Pack<T>*>(kt + voff - TL::URS);
+                kup = *reinterpret_cast<const Pack<T>*>(kt + voff + TL::URS);
+            }
+        }
+        const T vl = vt[voff - 1], vr = vt[voff + VEC];
+        T kl = T(0), kr = T(0);
+        if (VAR) { kl = kt[voff - 1]; kr = kt[voff + VEC]; }
+        const Pack<T> fv = *reinterpret_cast<const Pack<T>*>(fs(sc) + foff);
+        Pack<T> out;
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) {
+            const T vc = cur.v[j];
+            const T xm = j == 0 ? vl : cur.v[j - 1 < 0 ? 0 : j - 1];
+            const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+            T Av;
+            if (!VAR) {
+                T s = T(0);
+                s += prv.v[j] + nxt.v[j];
+                if (ND == 3) s += dn.v[j] + up.v[j];
+                s += xm + xp;
+                Av = (cf.twod * vc - s) * cf.ih2;
+            } else {
+                const T kc = kcur.v[j];
+                const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
+                const T kxp = j == VEC - 1 ? kr : kcur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+                T acc = T(0);
+                acc += kface(kc, kprv.v[j]) * (vc - prv.v[j]);
+                acc += kface(kc, knxt.v[j]) * (vc - nxt.v[j]);
+                if (ND == 3) {
+                    acc += kface(kc, kdn.v[j]) * (vc - dn.v[j]);
+                    acc += kface(kc, kup.v[j]) * (vc - up.v[j]);
+                }
+                acc += kface(kc, kxm) * (vc - xm);
+                acc += kface(kc, kxp) * (vc - xp);
+                Av = acc * cf.ih2;
+            }
+            out.v[j] = xin[j] ? fv.v[j] - Av : T(0);
+        }
+        *reinterpret_cast<Pack<T>*>(rring + (i & (TL::NR - 1)) * TL::RPLANE + foff) = out;
+        if (owned && z < me) {
+            if (r) *reinterpret_cast<Pack<T>*>(r + c) = out;
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) sq += double(out.v[j]) * double(out.v[j]);
+        }
+        __syncthreads();
+        if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
+        prv = cur; cur = nxt;
+        if (VAR) { kprv = kcur; kcur = knxt; }
+        if (gc != nullptr && i >= 3 && (i & 1)) {
+            // coarse plane Z = (z-1)/2 from r planes z-2, z-1, z (ring slots i-2, i-1, i)
+            const int Z = (z - 1) >> 1;
+            constexpr int CPR = TL::OWN / 2;                       // coarse nodes per row segment
+            constexpr int NCO = CPR * (ND == 3 ? TL::TY / 2 : TL::WX);
+            for (int n = tid; n < NCO; n += TL::NW * 32) {
+                const int q = n / CPR, Xl = n - q * CPR;
+                int X, Y, R0;
+                if (ND == 3) { X = (x0 >> 1) + Xl; Y = (y0 >> 1) + q; R0 = 2 * q + 1; }
+                else { X = ((x0 + q * TL::OWN) >> 1) + Xl; Y = Z; R0 = q; }
+                const bool cin = X >= 1 && X <= gcg.nx - 2 && (ND == 2 || (Y >= 1 && Y <= gcg.ny - 2));
+                if (!cin) continue;
+                const int e0 = 2 * Xl + VEC;
+                T acc = T(0);
+#pragma unroll
+                for (int dm = -1; dm <= 1; ++dm) {
+                    const T* rp = rring + ((i - 1 + dm) & (TL::NR - 1)) * TL::RPLANE;
+#pragma unroll
+                    for (int dy = (ND == 3 ? -1 : 0); dy <= (ND == 3 ? 1 : 0); ++dy)
+#pragma unroll
+                        for (int dx = -1; dx <= 1; ++dx) {
+                            const int m1 = (dm != 0) + (dy != 0) + (dx != 0);
+                            const T wgt = T(1.0 / double(1 << (ND + m1)));
+                            acc += wgt * rp[(R0 + dy) * TL::SEG + e0 + dx];
+                        }
+                }
+                gc[ND == 3 ? lidx(gcg, X, Y, Z) : lidx(gcg, X, Z, 0)] = acc;
+            }
+        }
+    }
+    const double t = block_sum(sq);
+    if (tid == 0) partial[bid] = t;
+}
+
 }  // namespace homg
