@@ -53,6 +53,10 @@ Coef<T> make_coef(const homg_solver* s, int m) {
     c.w = T(s->omega);
     c.twod = T(2 * s->ndim);
     c.w_over_D = c.w / (c.twod * c.ih2);
+    volatile T d = c.twod * c.ih2;          // one rounding, as on the device
+    c.D = d;
+    volatile T rd = T(1) / d;               // IEEE division: RN(1/D)
+    c.rD = rd;
     return c;
 }
 

@@ -21,6 +21,19 @@ struct alignas(16) Pack {
     T v[16 / sizeof(T)];
 };
 
+// x / D for a per-level constant D with rD = RN(1/D) precomputed on the host: q = RN(x rD),
+// r = x - q D (exact in one FMA), result RN(q + r rD).  By Markstein's theorem this is the correctly
+// rounded quotient, i.e. bit-identical to the IEEE division the generic kernels and the oracle
+// perform, at 3 instructions instead of a division sequence (tests: tiled == generic bitwise).
+__device__ __forceinline__ float div_const(float x, float D, float rD) {
+    const float q = x * rD;
+    return __fmaf_rn(__fmaf_rn(-q, D, x), rD, q);
+}
+__device__ __forceinline__ double div_const(double x, double D, double rD) {
+    const double q = x * rD;
+    return __fma_rn(__fma_rn(-q, D, x), rD, q);
+}
+
 template <class T, int ND>
 struct Tile {
     static constexpr int VEC = 16 / int(sizeof(T));
@@ -75,7 +88,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     const int count = me - ms + 2;                       // planes ms-1 .. me
 
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // keeps the shared address space
     __shared__ uint64_t bars[TL::NST];
     auto vs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
     auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES); };
@@ -157,12 +170,11 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
             const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
             T Av, D;
             if (!VAR) {
-                T s = T(0);
-                s += prv.v[j] + nxt.v[j];
+                T s = prv.v[j] + nxt.v[j];
                 if (ND == 3) s += dn.v[j] + up.v[j];
                 s += xm + xp;
                 Av = (cf.twod * vc - s) * cf.ih2;
-                D = cf.twod * cf.ih2;
+                D = cf.D;
             } else {
                 const T kc = kcur.v[j];
                 const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
@@ -179,7 +191,8 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
                 Av = acc * cf.ih2;
                 D = ds * cf.ih2;
             }
-            out.v[j] = xin[j] ? vc + cf.w * (gv.v[j] - Av) / D : T(0);
+            const T num = cf.w * (gv.v[j] - Av);
+            out.v[j] = xin[j] ? vc + (VAR ? num / D : div_const(num, cf.D, cf.rD)) : T(0);
         }
         if (row_ok) {
             *reinterpret_cast<Pack<T>*>(vout + c) = out;
@@ -274,7 +287,7 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     const int count = mlast - ms + 3;                                  // u planes ms-1 .. mlast+1
 
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // keeps the shared address space
     __shared__ uint64_t bars[TL::NST];
     auto us = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
     auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES); };
@@ -359,8 +372,7 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
             const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
             T Av;
             if (!VAR) {
-                T s = T(0);
-                s += prv.v[j] + nxt.v[j];
+                T s = prv.v[j] + nxt.v[j];
                 if (ND == 3) s += dn.v[j] + up.v[j];
                 s += xm + xp;
                 Av = (cf.twod * vc - s) * cf.ih2;

@@ -15,6 +15,8 @@ struct Coef {            // per-level operator constants
     T w;                 // omega
     T w_over_D;          // omega / (2d/h_m^2)      (constant coefficient)
     T twod;              // 2d
+    T D;                 // 2d * (1/h_m^2), rounded as the kernels round it (constant coefficient)
+    T rD;                // RN(1/D)
 };
 
 }  // namespace homg
