@@ -11,6 +11,8 @@
 // The arithmetic is the expression tree of homg_kernels.cuh (R14) — results are bit-identical
 // to the generic kernels and to the oracle.
 #pragma once
+#include <type_traits>
+
 #include "homg_kernels.cuh"
 #include "homg_tma.cuh"
 
@@ -20,6 +22,13 @@ template <class T>
 struct alignas(16) Pack {
     T v[16 / sizeof(T)];
 };
+
+template <class T>
+struct alignas(2 * sizeof(T)) HalfPack {
+    T v[2];
+};
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 // x / D for a per-level constant D with rD = RN(1/D) precomputed on the host: q = RN(x rD),
 // r = x - q D (exact in one FMA), result RN(q + r rD).  By Markstein's theorem this is the correctly
@@ -142,8 +151,10 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     if (tid == 0 && TL::NST < count) issue(TL::NST);
 
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
-    for (int i = 1; i <= count - 2; ++i, c += mstride) {
-        const int sn = (i + 1) & (TL::NST - 1), sc = i & (TL::NST - 1);
+    // one plane; K = (i-1) mod 4 is a compile-time constant so that every stage address is an immediate
+    auto step = [&](auto KC, const int i) {
+        constexpr int K = decltype(KC)::value;
+        constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
         nxt = *reinterpret_cast<const Pack<T>*>(vs(sn) + voff);
         if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
@@ -218,6 +229,16 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
         if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
         prv = cur; cur = nxt;
         if (VAR) { kprv = kcur; kcur = knxt; }
+        c += mstride;
+    };
+    for (int i = 1; i <= count - 2; i += 4) {
+        step(std::integral_constant<int, 0>{}, i);
+        if (i + 1 > count - 2) break;
+        step(std::integral_constant<int, 1>{}, i + 1);
+        if (i + 2 > count - 2) break;
+        step(std::integral_constant<int, 2>{}, i + 2);
+        if (i + 3 > count - 2) break;
+        step(std::integral_constant<int, 3>{}, i + 3);
     }
 }
 
@@ -343,9 +364,10 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
 
     double sq = 0.0;
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
-    for (int i = 1; i <= count - 2; ++i, c += mstride) {
+    auto step = [&](auto KC, const int i) {
+        constexpr int K = decltype(KC)::value;
         const int z = ms - 1 + i;
-        const int sn = (i + 1) & (TL::NST - 1), sc = i & (TL::NST - 1);
+        constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
         nxt = *reinterpret_cast<const Pack<T>*>(us(sn) + voff);
         if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
@@ -393,17 +415,18 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
             }
             out.v[j] = xin[j] ? fv.v[j] - Av : T(0);
         }
-        *reinterpret_cast<Pack<T>*>(rring + (i & (TL::NR - 1)) * TL::RPLANE + foff) = out;
+        *reinterpret_cast<Pack<T>*>(rring + ((K + 1) & (TL::NR - 1)) * TL::RPLANE + foff) = out;
         if (owned && z < me) {
             if (r) *reinterpret_cast<Pack<T>*>(r + c) = out;
 #pragma unroll
-            for (int j = 0; j < VEC; ++j) sq += double(out.v[j]) * double(out.v[j]);
+            for (int j = 0; j < VEC; ++j) { const double rv = double(out.v[j]); sq = __fma_rn(rv, rv, sq); }
         }
         __syncthreads();
         if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
         prv = cur; cur = nxt;
         if (VAR) { kprv = kcur; kcur = knxt; }
-        if (gc != nullptr && i >= 3 && (i & 1)) {
+        c += mstride;
+        if ((K & 1) == 0 && gc != nullptr && i >= 3) {
             // coarse plane Z = (z-1)/2 from r planes z-2, z-1, z (ring slots i-2, i-1, i)
             const int Z = (z - 1) >> 1;
             constexpr int CPR = TL::OWN / 2;                       // coarse nodes per row segment
@@ -416,22 +439,34 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
                 const bool cin = X >= 1 && X <= gcg.nx - 2 && (ND == 2 || (Y >= 1 && Y <= gcg.ny - 2));
                 if (!cin) continue;
                 const int e0 = 2 * Xl + VEC;
+                // weights are powers of two, so fma(w, r, acc) == acc + w*r bit for bit (the product is exact)
                 T acc = T(0);
 #pragma unroll
                 for (int dm = -1; dm <= 1; ++dm) {
-                    const T* rp = rring + ((i - 1 + dm) & (TL::NR - 1)) * TL::RPLANE;
+                    const T* rp = rring + ((K + dm) & (TL::NR - 1)) * TL::RPLANE;
 #pragma unroll
-                    for (int dy = (ND == 3 ? -1 : 0); dy <= (ND == 3 ? 1 : 0); ++dy)
-#pragma unroll
-                        for (int dx = -1; dx <= 1; ++dx) {
-                            const int m1 = (dm != 0) + (dy != 0) + (dx != 0);
-                            const T wgt = T(1.0 / double(1 << (ND + m1)));
-                            acc += wgt * rp[(R0 + dy) * TL::SEG + e0 + dx];
-                        }
+                    for (int dy = (ND == 3 ? -1 : 0); dy <= (ND == 3 ? 1 : 0); ++dy) {
+                        const T* rr = rp + (R0 + dy) * TL::SEG + e0;           // e0 is even: 2 scalars are one aligned load
+                        const T rm = rr[-1];
+                        const HalfPack<T> rc = *reinterpret_cast<const HalfPack<T>*>(rr);
+                        const int m0 = (dm != 0) + (dy != 0);
+                        acc = fma_rn(T(1.0 / double(1 << (ND + m0 + 1))), rm, acc);
+                        acc = fma_rn(T(1.0 / double(1 << (ND + m0))), rc.v[0], acc);
+                        acc = fma_rn(T(1.0 / double(1 << (ND + m0 + 1))), rc.v[1], acc);
+                    }
                 }
                 gc[ND == 3 ? lidx(gcg, X, Y, Z) : lidx(gcg, X, Z, 0)] = acc;
             }
         }
+    };
+    for (int i = 1; i <= count - 2; i += 4) {
+        step(std::integral_constant<int, 0>{}, i);
+        if (i + 1 > count - 2) break;
+        step(std::integral_constant<int, 1>{}, i + 1);
+        if (i + 2 > count - 2) break;
+        step(std::integral_constant<int, 2>{}, i + 2);
+        if (i + 3 > count - 2) break;
+        step(std::integral_constant<int, 3>{}, i + 3);
     }
     const double t = block_sum(sq);
     if (tid == 0) partial[bid] = t;
