@@ -4,8 +4,10 @@
 #include "homg_exec.h"
 
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 
-#include "homg_fused.cuh"
+#include "homg_first.cuh"
 
 namespace homg {
 
@@ -24,6 +26,11 @@ struct Rec {                 // bookkeeping while recording
     void check(int tag) {
         last_tag = tag;
         cudaError_t e = cudaPeekAtLastError();
+        static const bool dbg = std::getenv("HOMG_DEBUG_SYNC") != nullptr;   // localise a faulting launch
+        if (dbg && e == cudaSuccess) {
+            e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) std::fprintf(stderr, "homg: launch %d (tag %d) failed: %s\n", launches, tag, cudaGetErrorString(e));
+        }
         if (err == cudaSuccess && e != cudaSuccess) err = e;
         ++launches;
         if (ev) {
@@ -132,6 +139,39 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
     }
 }
 
+
+// first sweep of a visit on a tiled level t reached from level t+1 for the first time in the cycle:
+// interpolate + correct + relax in one pass (v0 is never written).
+template <class T, int ND, bool VAR>
+void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) {
+    homg_solver* s = R.s;
+    Level& Lt = s->L[t];
+    Level& Lc = s->L[t + 1];
+    using TL = FirstTile<T, ND>;
+    CUtensorMap tme, tma_, tmg, tmk;
+    bool ok = make_tmap<T, ND>(s, &tme, ec, Lc.g, TL::CW, ND == 3 ? TL::CROWS : 1) &&
+              make_tmap<T, ND>(s, &tma_, ac, Lc.g, TL::CW, ND == 3 ? TL::CROWS : 1) &&
+              make_tmap<T, ND>(s, &tmg, Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
+    if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, Lt.k, Lt.g, TL::FW, ND == 3 ? TL::TY + 2 : 1);
+    else tmk = tmg;
+    if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
+    const LevelGeom& g = Lt.g;
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const int interior = std::max(NM - 2, 1);
+    long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
+    int mc = s->march_chunk;
+    if (mc <= 0) {
+        long long nch = std::max<long long>(1, (long long)s->sm_count * 3 / std::max<long long>(tiles, 1));
+        mc = std::max(int((interior + nch - 1) / nch), 8);
+    }
+    mc = (mc + 1) & ~1;
+    int nch = (interior + mc - 1) / mc;
+    dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
+    k_relax_first<T, ND, VAR><<<grid, TL::NW * 32, first_smem_bytes<T, ND, VAR>(), R.st>>>(
+        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), vout, u, mc,
+        std::getenv("HOMG_DBG_FIRST") ? std::atoi(std::getenv("HOMG_DBG_FIRST")) : 0);
+}
+
 // S1 (+S5, + first step of S2 when `restrict1`): r = f - A u, ||r||^2 -> history / scalar, g_1 = P r.
 // Returns true when g_1 was written by the fused kernel.
 template <class T, int ND, bool VAR>
@@ -206,6 +246,8 @@ void rec_cycle(Rec& R) {
         const int t = s->sched_lv[vi], eta = s->sched_it[vi];
         Level& Lt = L[t];
         bool have_d0 = false;
+        bool fuse_first = false;
+        const T* fuse_ec = nullptr;
         if (cur < 0) {
             cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
             R.check(TAG_OTHER);
@@ -217,6 +259,13 @@ void rec_cycle(Rec& R) {
                     Level& Lc = L[m];
                     Level& Lf = L[m - 1];
                     int ef_assign = Lf.touched ? 0 : 1;
+                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && s->fuse_first) {
+                        fuse_first = true;                   // S3a of this hop happens inside the first sweep
+                        fuse_ec = rotp<T>(Lc, Lc.e);
+                        Lf.touched = true;
+                        a_zero[m] = 1;
+                        break;
+                    }
                     int af_mode = (m - 1 >= 1) ? (a_zero[m - 1] ? 2 : 1) : 0;
                     const T* ac = a_zero[m] ? nullptr : (const T*)Lc.a;
                     if (af_mode == 2 && !ac) af_mode = 0;          // 0 + 0: a stays "known zero"
@@ -280,6 +329,14 @@ void rec_cycle(Rec& R) {
             bool last = (it == eta - 1);
             bool book = last && t >= 1;
             bool addu = last && vi == nv - 1;
+            if (fuse_first && it == 0) {
+                launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
+                R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
+                R.acct(t + 1, 2.0);
+                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 2.0 : 0.0));
+                prev2 = prev_in; prev_in = in; in = out;
+                continue;
+            }
             launch_relax<T, ND, VAR>(R, t, rotp<T>(Lt, in), rotp<T>(Lt, out), book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0,
                                      have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
             R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
@@ -346,6 +403,9 @@ template <class T, int ND, bool VAR>
 cudaError_t set_attr() {
     cudaError_t e = cudaFuncSetAttribute(k_relax_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          relax_smem_bytes<T, ND, VAR>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_relax_first<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             first_smem_bytes<T, ND, VAR>());
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_res_tma<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 res_smem_bytes<T, ND, VAR>());
