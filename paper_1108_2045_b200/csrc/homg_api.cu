@@ -97,7 +97,10 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     s->omega = o.omega > 0 ? o.omega : (ndim == 2 ? 4.0 / 5.0 : 6.0 / 7.0);
     s->h = o.h > 0 ? o.h : 1.0 / double(dims[0] - 1);
     s->max_iters = o.max_iters > 0 ? o.max_iters : 4;
-    s->coarse_threshold = o.coarse_threshold_nodes;
+    s->coarse_threshold = o.coarse_threshold_nodes > 0 ? o.coarse_threshold_nodes
+                                                       : (o.coarse_threshold_nodes < 0 ? 0 : kCoarseNodesDefault);
+    if (const char* ev = std::getenv("HOMG_COARSE_NODES")) s->coarse_threshold = std::atoll(ev);
+    if (const char* ev = std::getenv("HOMG_COARSE_CLUSTER")) s->coarse_cluster = std::atoi(ev);
     s->use_graph = o.use_graph != 0;
     s->tiled_min_nodes = o.tiled_min_nodes > 0 ? o.tiled_min_nodes : (o.tiled_min_nodes < 0 ? -1 : kTiledMinNodesDefault);
     if (const char* ev = std::getenv("HOMG_TILED_MIN_NODES")) s->tiled_min_nodes = std::atoll(ev);
@@ -183,6 +186,7 @@ homg_status homg_cycle(homg_solver* s, int n) {
     if (n < 0) return set_err(s, HOMG_EINVAL, "n < 0");
     if (!s->have_rhs) return set_err(s, HOMG_ESTATE, "homg_cycle before homg_set_rhs");
     if (s->var && !s->have_coef) return set_err(s, HOMG_ESTATE, "homg_cycle before homg_set_coefficient");
+    CU(s, exec_prepare(s));
     if (s->use_graph && !s->graph_exec) {
         // capture one cycle on the private stream (capturing does not execute anything)
         CU(s, cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
@@ -250,6 +254,7 @@ homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* l
     if (!ms_by_tag || !launches_by_tag || !bytes_by_tag || cap < HOMG_TAG_COUNT) return set_err(s, HOMG_EINVAL, "profile arrays too small");
     if (!s->have_rhs || (s->var && !s->have_coef)) return set_err(s, HOMG_ESTATE, "profile before set_rhs / set_coefficient");
     for (int i = 0; i < cap; ++i) { ms_by_tag[i] = 0.0; launches_by_tag[i] = 0; bytes_by_tag[i] = 0.0; }
+    CU(s, exec_prepare(s));
     for (int c = 0; c < n; ++c) CU(s, exec_cycle_profiled(s, s->stream, ms_by_tag, launches_by_tag, bytes_by_tag));
     s->cycles_issued += n;
     return HOMG_OK;
@@ -282,6 +287,7 @@ void homg_destroy(homg_solver* s) {
     if (!s) return;
     drop_graph(s);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    if (s->prog_dev) cudaFree(s->prog_dev);
     delete s;
 }
 

@@ -7,11 +7,16 @@
 #include <cstdio>
 #include <cstdlib>
 
+#include <cstring>
+
+#include "homg_coarse.cuh"
 #include "homg_first.cuh"
 
 namespace homg {
 
 namespace {
+
+constexpr long long kTinyNodes = 800;   // <= 9^3, 28^2: one CTA works the level (one SM's load bandwidth suffices)
 
 struct Rec {                 // bookkeeping while recording
     homg_solver* s;
@@ -23,8 +28,24 @@ struct Rec {                 // bookkeeping while recording
     std::vector<int>* ev_tag = nullptr;
     int last_tag = TAG_OTHER;
     double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class
+    bool plan = false;                        // planning pass: build the coarse program, launch nothing
+    std::vector<unsigned char> prog;          // CoarseOp records of the whole cycle, in order
+    int prog_nops = 0, run_begin = 0, run_len = 0;
+    long long run_maxnodes = 0;
+    template <class OP>
+    void push(const OP& o, long long nodes) {
+        const unsigned char* b = reinterpret_cast<const unsigned char*>(&o);
+        prog.insert(prog.end(), b, b + sizeof(OP));
+        if (run_len == 0) { run_begin = prog_nops; run_maxnodes = 0; }
+        // `act` sits right after `type` in every CoarseOp<T>
+        reinterpret_cast<int*>(prog.data() + prog.size() - sizeof(OP))[1] = nodes <= kTinyNodes ? 1 : 0;
+        ++prog_nops; ++run_len;
+        if (nodes > run_maxnodes) run_maxnodes = nodes;
+    }
+    void acct(int level, double arrays, int tag) { last_tag = tag; acct(level, arrays); }
     void check(int tag) {
         last_tag = tag;
+        if (plan) return;
         cudaError_t e = cudaPeekAtLastError();
         static const bool dbg = std::getenv("HOMG_DEBUG_SYNC") != nullptr;   // localise a faulting launch
         if (dbg && e == cudaSuccess) {
@@ -172,6 +193,35 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
         std::getenv("HOMG_DBG_FIRST") ? std::atoi(std::getenv("HOMG_DBG_FIRST")) : 0);
 }
 
+
+// launches the pending run of coarse-level operations as ONE cluster (K_coarse)
+template <class T, int ND, bool VAR>
+void flush_run(Rec& R) {
+    if (R.run_len == 0) return;
+    homg_solver* s = R.s;
+    if (!R.plan) {
+        int ncta = R.run_maxnodes <= kTinyNodes ? 1 : 8;
+        if (s->coarse_cluster > 0) ncta = s->coarse_cluster;
+        for (int b = 0; b < R.run_len; b += kMaxRunOps) {       // long runs: kMaxRunOps records per launch
+            const int n = std::min(kMaxRunOps, R.run_len - b);
+            const CoarseOp<T>* dev = static_cast<const CoarseOp<T>*>(s->prog_dev) + R.run_begin + b;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(ncta, 1, 1);
+            cfg.blockDim = dim3(1024, 1, 1);
+            cfg.stream = R.st;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = ncta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            cudaError_t e = ncta > 1 ? cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, true>, dev, n)
+                                     : cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, false>, dev, n);
+            if (R.err == cudaSuccess && e != cudaSuccess) R.err = e;
+            R.check(TAG_COARSE);
+        }
+    }
+    R.run_len = 0;
+}
+
 // S1 (+S5, + first step of S2 when `restrict1`): r = f - A u, ||r||^2 -> history / scalar, g_1 = P r.
 // Returns true when g_1 was written by the fused kernel.
 template <class T, int ND, bool VAR>
@@ -202,7 +252,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         int nch = (interior + mc - 1) / mc;
         dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
         n = int(grid.x * grid.y * grid.z);
-        k_res_tma<T, ND, VAR><<<grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), R.st>>>(
+        if (!R.plan) k_res_tma<T, ND, VAR><<<grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), R.st>>>(
             tmu, tmf, tmk, g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
             fused_restrict ? (T*)s->L[1].gsrc : nullptr, s->partial, mc);
         R.check(TAG_RESIDUAL0);
@@ -210,13 +260,13 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         if (fused_restrict) R.acct(1, 1.0);
     } else {
         dim3 g = grd(L0.g);
-        k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
+        if (!R.plan) k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
                                                        (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
         R.check(TAG_RESIDUAL0);
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
         n = int(g.x * g.y * g.z);
     }
-    k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
+    if (!R.plan) k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
                                         to_history ? 1 : 0, to_history ? nullptr : s->scalar);
     R.check(TAG_NORM_FINISH);
     return fused_restrict;
@@ -230,14 +280,29 @@ void rec_cycle(Rec& R) {
     for (auto& l : L) { l.e = 0; l.touched = false; l.vk = l.vkm1 = l.vkm2 = -1; l.eta_last = 0; }
     std::vector<char> a_zero(s->levels, 1);      // a_m == 0 (nothing pending)
     std::vector<char> dp_is_d0(s->levels, 0);    // eta == 1 visit: its dp is its own d0
+    auto small = [&](int m) { return s->coarse_threshold > 0 && L[m].n_nodes <= s->coarse_threshold; };
+    auto newop = [&](int type, int mo) {
+        CoarseOp<T> o;
+        std::memset(&o, 0, sizeof(o));
+        o.type = type; o.go = L[mo].g; o.gi = L[mo].g; o.gv = L[mo].g;
+        return o;
+    };
+    auto flush = [&]() { flush_run<T, ND, VAR>(R); };
 
     // S1: r = f - A u, ||r||^2 -> history
     const bool have_g1 = rec_norm<T, ND, VAR>(R, true, true, true);
     // S2: nested restriction g_m = P g_{m-1}
     for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
-        k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
-        R.check(TAG_RESTRICT);
-        R.acct(m - 1, 1.0); R.acct(m, 1.0);
+        if (small(m)) {
+            CoarseOp<T> o = newop(OP_RESTRICT, m);
+            o.gi = L[m - 1].g; o.p[0] = (const T*)L[m - 1].gsrc; o.q[0] = (T*)L[m].gsrc;
+            R.push(o, L[m].n_nodes);
+        } else {
+            flush();
+            if (!R.plan) k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
+            R.check(TAG_RESTRICT);
+        }
+        R.acct(m - 1, 1.0, small(m) ? TAG_COARSE : TAG_RESTRICT); R.acct(m, 1.0, small(m) ? TAG_COARSE : TAG_RESTRICT);
     }
     // S3: MFMG visits
     int cur = -1;
@@ -249,8 +314,15 @@ void rec_cycle(Rec& R) {
         bool fuse_first = false;
         const T* fuse_ec = nullptr;
         if (cur < 0) {
-            cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
-            R.check(TAG_OTHER);
+            if (small(t)) {
+                CoarseOp<T> o = newop(OP_ZERO, t);
+                o.count = (long long)Lt.n_alloc; o.q[0] = (T*)Lt.rot[Lt.e];
+                R.push(o, L[t].n_nodes);
+            } else {
+                flush();
+                if (!R.plan) cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
+                R.check(TAG_OTHER);
+            }
             Lt.touched = true;
         } else {
             if (t < cur) {
@@ -269,11 +341,20 @@ void rec_cycle(Rec& R) {
                     int af_mode = (m - 1 >= 1) ? (a_zero[m - 1] ? 2 : 1) : 0;
                     const T* ac = a_zero[m] ? nullptr : (const T*)Lc.a;
                     if (af_mode == 2 && !ac) af_mode = 0;          // 0 + 0: a stays "known zero"
-                    k_deliver<T, ND><<<grd(Lf.g), blk(), 0, R.st>>>(Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
-                                                                     rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
-                    R.check(m - 1 == 0 ? TAG_DELIVER0 : TAG_DELIVER);
-                    R.acct(m, ac ? 2.0 : 1.0);
-                    R.acct(m - 1, (ef_assign ? 1.0 : 2.0) + (af_mode == 1 ? 2.0 : af_mode == 2 ? 1.0 : 0.0));
+                    const int tag = small(m - 1) ? TAG_COARSE : (m - 1 == 0 ? TAG_DELIVER0 : TAG_DELIVER);
+                    if (small(m - 1)) {
+                        CoarseOp<T> o = newop(OP_DELIVER, m - 1);
+                        o.gi = Lc.g; o.p[0] = rotp<T>(Lc, Lc.e); o.p[1] = ac; o.q[0] = rotp<T>(Lf, Lf.e); o.q[1] = (T*)Lf.a;
+                        o.f0 = ef_assign; o.f1 = af_mode;
+                        R.push(o, Lf.n_nodes);
+                    } else {
+                        flush();
+                        if (!R.plan) k_deliver<T, ND><<<grd(Lf.g), blk(), 0, R.st>>>(Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
+                                                                                    rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
+                        R.check(tag);
+                    }
+                    R.acct(m, ac ? 2.0 : 1.0, tag);
+                    R.acct(m - 1, (ef_assign ? 1.0 : 2.0) + (af_mode == 1 ? 2.0 : af_mode == 2 ? 1.0 : 0.0), tag);
                     Lf.touched = true;
                     if (af_mode) a_zero[m - 1] = 0;
                     a_zero[m] = 1;                                  // a_m delivered
@@ -281,10 +362,18 @@ void rec_cycle(Rec& R) {
             } else if (t > cur) {
                 // S3b inject level m-1 -> m (same memory cells in the paper's single array)
                 for (int m = cur + 1; m <= t; ++m) {
-                    k_inject<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
-                                                                      rotp<T>(L[m], L[m].e));
-                    R.check(TAG_INJECT);
-                    R.acct(m, 2.0);
+                    const int tag = small(m) ? TAG_COARSE : TAG_INJECT;
+                    if (small(m)) {
+                        CoarseOp<T> o = newop(OP_INJECT, m);
+                        o.gi = L[m - 1].g; o.p[0] = rotp<T>(L[m - 1], L[m - 1].e); o.q[0] = rotp<T>(L[m], L[m].e);
+                        R.push(o, L[m].n_nodes);
+                    } else {
+                        flush();
+                        if (!R.plan) k_inject<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
+                                                                                     rotp<T>(L[m], L[m].e));
+                        R.check(tag);
+                    }
+                    R.acct(m, 2.0, tag);
                     L[m].touched = true;
                 }
             }
@@ -294,19 +383,36 @@ void rec_cycle(Rec& R) {
                 const T* X = rotp<T>(Lv, Lv.vk);
                 const T* Y = rotp<T>(Lv, Lv.vkm1);
                 if (t >= cur) {
-                    k_d0_up<T, ND><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
-                    R.check(TAG_D0);
-                    R.acct(t, 3.0);
+                    const int tag = small(t) ? TAG_COARSE : TAG_D0;
+                    if (small(t)) {
+                        CoarseOp<T> o = newop(OP_D0_UP, t);
+                        o.gi = Lv.g; o.s = 1 << (t - cur); o.p[0] = X; o.p[1] = Y; o.q[0] = (T*)Lt.d0;
+                        R.push(o, Lt.n_nodes);
+                    } else {
+                        flush();
+                        if (!R.plan) k_d0_up<T, ND><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
+                        R.check(tag);
+                    }
+                    R.acct(t, 3.0, tag);
                 } else {
                     const T* A = dp_is_d0[cur] ? (const T*)Lv.d0 : rotp<T>(Lv, Lv.vkm1);
                     const T* B = dp_is_d0[cur] ? nullptr : rotp<T>(Lv, Lv.vkm2);
                     for (int m = cur; m > t; --m) {
                         bool last = (m - 1 == t);
                         T* out = last ? (T*)Lt.d0 : (T*)L[m - 1].tmp;
-                        k_d0_down<T, ND><<<grd(L[m - 1].g), blk(), 0, R.st>>>(L[m - 1].g, L[m].g, A, B, out,
-                                                                               last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
-                        R.check(TAG_D0);
-                        R.acct(m, B ? 2.0 : 1.0); R.acct(m - 1, 1.0);
+                        const int tag = small(m - 1) ? TAG_COARSE : TAG_D0;
+                        if (small(m - 1)) {
+                            CoarseOp<T> o = newop(OP_D0_DOWN, m - 1);
+                            o.gi = L[m].g; o.gv = Lv.g; o.s = last ? (1 << (cur - t)) : 0;
+                            o.p[0] = A; o.p[1] = B; o.p[2] = X; o.p[3] = Y; o.q[0] = out;
+                            R.push(o, L[m - 1].n_nodes);
+                        } else {
+                            flush();
+                            if (!R.plan) k_d0_down<T, ND><<<grd(L[m - 1].g), blk(), 0, R.st>>>(L[m - 1].g, L[m].g, A, B, out,
+                                                                                              last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
+                            R.check(tag);
+                        }
+                        R.acct(m, B ? 2.0 : 1.0, tag); R.acct(m - 1, 1.0, tag);
                         A = out; B = nullptr;
                     }
                 }
@@ -314,8 +420,15 @@ void rec_cycle(Rec& R) {
             }
         }
         if (t >= 1 && !have_d0 && eta == 1) {        // first visit with eta = 1: its dp is d0 = 0
-            cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st);
-            R.check(TAG_OTHER);
+            if (small(t)) {
+                CoarseOp<T> o = newop(OP_ZERO, t);
+                o.count = (long long)Lt.n_alloc; o.q[0] = (T*)Lt.d0;
+                R.push(o, Lt.n_nodes);
+            } else {
+                flush();
+                if (!R.plan) cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st);
+                R.check(TAG_OTHER);
+            }
             have_d0 = true;
         }
         // S3d eta damped-Jacobi sweeps; S3e bookkeeping fused into the last one; S4 u += e fused
@@ -329,19 +442,33 @@ void rec_cycle(Rec& R) {
             bool last = (it == eta - 1);
             bool book = last && t >= 1;
             bool addu = last && vi == nv - 1;
+            const int tag = small(t) ? TAG_COARSE : (t == 0 ? TAG_RELAX0 : TAG_RELAX);
             if (fuse_first && it == 0) {
-                launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
-                R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
-                R.acct(t + 1, 2.0);
-                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 2.0 : 0.0));
+                flush();
+                if (!R.plan) launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
+                R.check(tag);
+                R.acct(t + 1, 2.0, tag);
+                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 2.0 : 0.0), tag);
                 prev2 = prev_in; prev_in = in; in = out;
                 continue;
             }
-            launch_relax<T, ND, VAR>(R, t, rotp<T>(Lt, in), rotp<T>(Lt, out), book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0,
-                                     have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
-            R.check(t == 0 ? TAG_RELAX0 : TAG_RELAX);
+            if (small(t)) {
+                CoarseOp<T> o = newop(OP_RELAX, t);
+                o.cf = make_coef<T>(s, t);
+                o.p[0] = rotp<T>(Lt, in); o.p[1] = (const T*)Lt.gsrc; o.p[2] = (const T*)Lt.k;
+                o.p[3] = have_d0 ? (const T*)Lt.d0 : nullptr; o.p[4] = rotp<T>(Lt, v0);
+                o.q[0] = rotp<T>(Lt, out); o.q[1] = book ? (T*)Lt.a : nullptr; o.q[2] = addu ? (T*)s->u : nullptr;
+                o.f0 = a_zero[t] ? 1 : 0;
+                R.push(o, Lt.n_nodes);
+            } else {
+                flush();
+                if (!R.plan)
+                    launch_relax<T, ND, VAR>(R, t, rotp<T>(Lt, in), rotp<T>(Lt, out), book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0,
+                                             have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
+                R.check(tag);
+            }
             R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
-                          (addu ? 2.0 : 0.0));
+                          (addu ? 2.0 : 0.0), tag);
             prev2 = prev_in; prev_in = in; in = out;
         }
         if (t >= 1) a_zero[t] = 0;
@@ -349,6 +476,7 @@ void rec_cycle(Rec& R) {
         dp_is_d0[t] = (eta == 1);
         cur = t;
     }
+    flush();
 }
 
 template <class T, int ND, bool VAR>
@@ -430,6 +558,22 @@ cudaError_t exec_init(homg_solver* s) {
     if ((e = set_attr<double, 2, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, true>()) != cudaSuccess) return e;
+    return cudaSuccess;
+}
+
+cudaError_t exec_prepare(homg_solver* s) {
+    if (s->prog_ready) return cudaSuccess;
+    Rec P{s, s->stream};
+    P.plan = true;
+    HOMG_DISPATCH(s, rec_cycle, P);
+    if (P.err != cudaSuccess) return P.err;
+    if (!P.prog.empty()) {
+        cudaError_t e = cudaMalloc(&s->prog_dev, P.prog.size());
+        if (e != cudaSuccess) return e;
+        e = cudaMemcpy(s->prog_dev, P.prog.data(), P.prog.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return e;
+    }
+    s->prog_ready = true;
     return cudaSuccess;
 }
 

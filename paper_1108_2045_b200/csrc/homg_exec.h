@@ -15,6 +15,14 @@ constexpr long long kTiledMinNodesDefault = 200000;   // 65^3 and up, 449^2 and 
 // Device queries, the driver's tensor-map encoder, kernel attributes.  Called once by homg_create.
 cudaError_t exec_init(homg_solver* s);
 
+// measured on cfg2 (profiles/): one-CTA runs pay off up to 9^3; a 17^3 / 33^3 operation needs more load
+// bandwidth than a few SMs have, so those levels keep one launch per operation
+constexpr long long kCoarseNodesDefault = 800;
+
+// Builds the coarse-level program of one cycle (planning pass, no launches) and uploads it to a
+// small library-owned device buffer.  Must run before exec_cycle and outside stream capture.
+cudaError_t exec_prepare(homg_solver* s);
+
 // Issues the launches of ONE outer cycle on `st` (which may be a capturing stream) and fills
 // s->launches_per_cycle / s->bytes_cycle_*.
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st);

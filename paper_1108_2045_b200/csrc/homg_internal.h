@@ -61,7 +61,10 @@ struct homg_solver {
     bool var = false;
     double omega = 0, h = 0;
     int max_iters = 4;
-    int coarse_threshold = 0;
+    long long coarse_threshold = 0;  // levels with <= this many nodes run inside K_coarse launches
+    int coarse_cluster = 0;          // 0: automatic cluster size (1, 4 or 8 CTAs)
+    void* prog_dev = nullptr;        // CoarseOp records of one cycle (library-owned device memory)
+    bool prog_ready = false;
     bool use_graph = true;
     long long tiled_min_nodes = 0;   // levels with >= this many nodes use the TMA-tiled kernels
     int march_chunk = 0;             // 0: automatic
