@@ -106,6 +106,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (const char* ev = std::getenv("HOMG_TILED_MIN_NODES")) s->tiled_min_nodes = std::atoll(ev);
     s->march_chunk = o.march_chunk > 0 ? o.march_chunk : 0;
     if (const char* ev = std::getenv("HOMG_MARCH_CHUNK")) s->march_chunk = std::atoi(ev);
+    if (const char* ev = std::getenv("HOMG_PDL")) s->pdl = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);
     s->hist_cap = hist_cap;

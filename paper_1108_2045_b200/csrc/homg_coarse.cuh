@@ -183,6 +183,7 @@ __device__ __forceinline__ void coarse_node(const CoarseOp<T>& o, int x, int y, 
 // separated by a CTA barrier; everything else by the whole cluster and a cluster barrier.
 template <class T, int ND, bool VAR, bool MULTI>
 __global__ void __launch_bounds__(1024) k_coarse_run(const CoarseOp<T>* __restrict__ ops, int nops) {
+    pdl_start();
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     __shared__ CoarseOp<T> sops[kMaxRunOps];

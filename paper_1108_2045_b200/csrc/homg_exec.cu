@@ -70,6 +70,23 @@ struct Rec {                 // bookkeeping while recording
     }
 };
 
+
+// every kernel is launched with programmatic stream serialization (PDL): the next kernel of the
+// stream / graph may start while this one drains; each kernel executes griddepcontrol.wait before
+// its first global access (pdl_start() in homg_kernels.cuh), so data dependences are unchanged.
+template <class K, class... Args>
+void klaunch(Rec& R, K kern, dim3 grid, dim3 block, size_t smem, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = R.st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = R.s->pdl ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
+    if (R.err == cudaSuccess && e != cudaSuccess) R.err = e;
+}
+inline dim3 d3(int x) { return dim3(x, 1, 1); }
+
 inline dim3 blk() { return dim3(32, 8, 1); }
 inline dim3 grd(const LevelGeom& g) { return dim3((g.nx + 31) / 32, (g.ny + 7) / 8, g.nz); }
 
@@ -152,10 +169,10 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
         int nch = 1;
         int mc = march_chunk<T, ND>(s, Lt.g, &nch);
         dim3 grid((Lt.g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (Lt.g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
-        k_relax_tma<T, ND, VAR><<<grid, 256, relax_smem_bytes<T, ND, VAR>(), R.st>>>(tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
+        klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
                                                                                       d0, v0, u, mc);
     } else {
-        k_relax<T, ND, VAR><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, cf, vin, (const T*)Lt.gsrc, (const T*)Lt.k, vout, a,
+        klaunch(R, k_relax<T, ND, VAR>, grd(Lt.g), blk(), 0, Lt.g, cf, vin, (const T*)Lt.gsrc, (const T*)Lt.k, vout, a,
                                                             a_assign, d0, v0, u);
     }
 }
@@ -188,9 +205,8 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
     mc = (mc + 1) & ~1;
     int nch = (interior + mc - 1) / mc;
     dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
-    k_relax_first<T, ND, VAR><<<grid, TL::NW * 32, first_smem_bytes<T, ND, VAR>(), R.st>>>(
-        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), vout, u, mc,
-        std::getenv("HOMG_DBG_FIRST") ? std::atoi(std::getenv("HOMG_DBG_FIRST")) : 0);
+    klaunch(R, k_relax_first<T, ND, VAR>, grid, TL::NW * 32, first_smem_bytes<T, ND, VAR>(), 
+        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), vout, u, mc);
 }
 
 
@@ -209,10 +225,12 @@ void flush_run(Rec& R) {
             cfg.gridDim = dim3(ncta, 1, 1);
             cfg.blockDim = dim3(1024, 1, 1);
             cfg.stream = R.st;
-            cudaLaunchAttribute at[1];
+            cudaLaunchAttribute at[2];
             at[0].id = cudaLaunchAttributeClusterDimension;
             at[0].val.clusterDim.x = ncta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-            cfg.attrs = at; cfg.numAttrs = 1;
+            at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            at[1].val.programmaticStreamSerializationAllowed = s->pdl ? 1 : 0;
+            cfg.attrs = at; cfg.numAttrs = 2;
             cudaError_t e = ncta > 1 ? cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, true>, dev, n)
                                      : cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, false>, dev, n);
             if (R.err == cudaSuccess && e != cudaSuccess) R.err = e;
@@ -252,7 +270,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         int nch = (interior + mc - 1) / mc;
         dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
         n = int(grid.x * grid.y * grid.z);
-        if (!R.plan) k_res_tma<T, ND, VAR><<<grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), R.st>>>(
+        if (!R.plan) klaunch(R, k_res_tma<T, ND, VAR>, grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), 
             tmu, tmf, tmk, g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
             fused_restrict ? (T*)s->L[1].gsrc : nullptr, s->partial, mc);
         R.check(TAG_RESIDUAL0);
@@ -260,13 +278,13 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         if (fused_restrict) R.acct(1, 1.0);
     } else {
         dim3 g = grd(L0.g);
-        if (!R.plan) k_residual<T, ND, VAR><<<g, blk(), 0, R.st>>>(L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
+        if (!R.plan) klaunch(R, k_residual<T, ND, VAR>, g, blk(), 0, L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
                                                        (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
         R.check(TAG_RESIDUAL0);
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
         n = int(g.x * g.y * g.z);
     }
-    if (!R.plan) k_norm_finish<<<1, 256, 0, R.st>>>(s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
+    if (!R.plan) klaunch(R, k_norm_finish, 1, 256, 0, s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
                                         to_history ? 1 : 0, to_history ? nullptr : s->scalar);
     R.check(TAG_NORM_FINISH);
     return fused_restrict;
@@ -299,7 +317,7 @@ void rec_cycle(Rec& R) {
             R.push(o, L[m].n_nodes);
         } else {
             flush();
-            if (!R.plan) k_restrict<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
+            if (!R.plan) klaunch(R, k_restrict<T, ND>, grd(L[m].g), blk(), 0, L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
             R.check(TAG_RESTRICT);
         }
         R.acct(m - 1, 1.0, small(m) ? TAG_COARSE : TAG_RESTRICT); R.acct(m, 1.0, small(m) ? TAG_COARSE : TAG_RESTRICT);
@@ -349,7 +367,7 @@ void rec_cycle(Rec& R) {
                         R.push(o, Lf.n_nodes);
                     } else {
                         flush();
-                        if (!R.plan) k_deliver<T, ND><<<grd(Lf.g), blk(), 0, R.st>>>(Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
+                        if (!R.plan) klaunch(R, k_deliver<T, ND>, grd(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
                                                                                     rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
                         R.check(tag);
                     }
@@ -369,7 +387,7 @@ void rec_cycle(Rec& R) {
                         R.push(o, L[m].n_nodes);
                     } else {
                         flush();
-                        if (!R.plan) k_inject<T, ND><<<grd(L[m].g), blk(), 0, R.st>>>(L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
+                        if (!R.plan) klaunch(R, k_inject<T, ND>, grd(L[m].g), blk(), 0, L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
                                                                                      rotp<T>(L[m], L[m].e));
                         R.check(tag);
                     }
@@ -390,7 +408,7 @@ void rec_cycle(Rec& R) {
                         R.push(o, Lt.n_nodes);
                     } else {
                         flush();
-                        if (!R.plan) k_d0_up<T, ND><<<grd(Lt.g), blk(), 0, R.st>>>(Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
+                        if (!R.plan) klaunch(R, k_d0_up<T, ND>, grd(Lt.g), blk(), 0, Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);
                         R.check(tag);
                     }
                     R.acct(t, 3.0, tag);
@@ -408,7 +426,7 @@ void rec_cycle(Rec& R) {
                             R.push(o, L[m - 1].n_nodes);
                         } else {
                             flush();
-                            if (!R.plan) k_d0_down<T, ND><<<grd(L[m - 1].g), blk(), 0, R.st>>>(L[m - 1].g, L[m].g, A, B, out,
+                            if (!R.plan) klaunch(R, k_d0_down<T, ND>, grd(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,
                                                                                               last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
                             R.check(tag);
                         }
@@ -483,7 +501,7 @@ template <class T, int ND, bool VAR>
 void rec_sample(Rec& R) {
     homg_solver* s = R.s;
     for (int m = 1; m < s->levels; ++m) {
-        k_sample_coef<T, ND><<<grd(s->L[m].g), blk(), 0, R.st>>>(s->L[m].g, s->L[m - 1].g, (const T*)s->L[m - 1].k,
+        klaunch(R, k_sample_coef<T, ND>, grd(s->L[m].g), blk(), 0, s->L[m].g, s->L[m - 1].g, (const T*)s->L[m - 1].k,
                                                                    (T*)s->L[m].k);
         R.check(TAG_OTHER);
     }
@@ -492,14 +510,14 @@ void rec_sample(Rec& R) {
 template <class T, int ND>
 void rec_pack(Rec& R, const void* dense, void* padded, int zero_boundary) {
     const LevelGeom& g = R.s->L[0].g;
-    k_pack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)dense, (T*)padded, zero_boundary);
+    klaunch(R, k_pack<T, ND>, grd(g), blk(), 0, g, (const T*)dense, (T*)padded, zero_boundary);
     R.check(TAG_OTHER);
 }
 
 template <class T, int ND>
 void rec_unpack(Rec& R, const void* padded, void* dense) {
     const LevelGeom& g = R.s->L[0].g;
-    k_unpack<T, ND><<<grd(g), blk(), 0, R.st>>>(g, (const T*)padded, (T*)dense);
+    klaunch(R, k_unpack<T, ND>, grd(g), blk(), 0, g, (const T*)padded, (T*)dense);
     R.check(TAG_OTHER);
 }
 

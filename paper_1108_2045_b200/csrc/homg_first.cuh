@@ -67,7 +67,8 @@ template <class T, int ND, bool VAR>
 __global__ void __launch_bounds__(FirstTile<T, ND>::NW * 32)
 k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ CUtensorMap tma_,
               const __grid_constant__ CUtensorMap tmg, const __grid_constant__ CUtensorMap tmk, LevelGeom g,
-              Coef<T> cf, T* __restrict__ vout, T* __restrict__ u, int mchunk, int dbg) {
+              Coef<T> cf, T* __restrict__ vout, T* __restrict__ u, int mchunk) {
+    pdl_start();
     using TL = FirstTile<T, ND>;
     constexpr int VEC = TL::VEC;
     constexpr int NCV = VEC / 2 + 1;
@@ -133,16 +134,9 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
             }
         }
     };
-    if (dbg == 1) return;
     if (tid == 0) {
-        if (dbg != 3) for (int zc = 0; zc < TL::NC && zc < ncz; ++zc) issue_c(zc);
-        if (dbg != 2) for (int q = 0; q < TL::NG && q < nq; ++q) issue_f(q);
-    }
-    if (dbg >= 2 && dbg <= 4) {
-        if (dbg != 3) for (int zc = 0; zc < TL::NC && zc < ncz; ++zc) mbar_wait(&cbar[zc], 0);
-        if (dbg != 2) for (int q = 0; q < TL::NG && q < nq; ++q) mbar_wait(&fbar[q], 0);
-        __syncthreads();
-        if (dbg != 4) return;
+        for (int zc = 0; zc < TL::NC && zc < ncz; ++zc) issue_c(zc);
+        for (int q = 0; q < TL::NG && q < nq; ++q) issue_f(q);
     }
 
     // ---- this thread's place ----
@@ -210,7 +204,6 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
 
     produce(0);
     if (nq > 1) produce(1);
-    if (dbg == 4) { __syncthreads(); return; }
     Pack<T> prv, cur, nxt, kprv, kcur, knxt;
     if (VAR) {
         mbar_wait(&fbar[0], 0);

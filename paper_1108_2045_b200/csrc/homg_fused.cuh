@@ -81,6 +81,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
             const __grid_constant__ CUtensorMap tmk, LevelGeom g, Coef<T> cf, T* __restrict__ vout,
             T* __restrict__ a, int a_assign, const T* __restrict__ d0, const T* __restrict__ v0,
             T* __restrict__ u, int mchunk) {
+    pdl_start();
     using TL = Tile<T, ND>;
     constexpr int VEC = TL::VEC;
     constexpr int STAGE = relax_stage_bytes<T, ND, VAR>();
@@ -289,6 +290,7 @@ __global__ void __launch_bounds__(ResTile<T, ND>::NW * 32)
 k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUtensorMap tmf,
           const __grid_constant__ CUtensorMap tmk, LevelGeom g, LevelGeom gcg, Coef<T> cf, T* __restrict__ r,
           T* __restrict__ gc, double* __restrict__ partial, int mchunk) {
+    pdl_start();
     using TL = ResTile<T, ND>;
     constexpr int VEC = TL::VEC;
     constexpr int STAGE = res_stage_bytes<T, ND, VAR>();

@@ -68,6 +68,7 @@ struct homg_solver {
     bool use_graph = true;
     long long tiled_min_nodes = 0;   // levels with >= this many nodes use the TMA-tiled kernels
     int march_chunk = 0;             // 0: automatic
+    bool pdl = true;                 // programmatic dependent launch on every kernel (HOMG_PDL=0 disables)
     bool fuse_first = true;          // fused interpolate+correct+relax first sweep (HOMG_FUSE_FIRST=0 disables)
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create

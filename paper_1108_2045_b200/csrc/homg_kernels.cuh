@@ -17,6 +17,14 @@
 
 namespace homg {
 
+// Programmatic dependent launch: let the next kernel of the stream begin its launch now, then wait
+// until every kernel before this one has completed and flushed its writes.  Must precede the first
+// global access of a kernel; a no-op when the launch carries no programmatic attribute.
+__device__ __forceinline__ void pdl_start() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ long long lidx(const LevelGeom& g, int x, int y, int z) {
     return (long long)z * g.pp + (long long)y * g.px + x;
 }
@@ -108,6 +116,7 @@ __device__ __forceinline__ double block_sum(double v) {
 template <class T, int ND, bool VAR>
 __global__ void k_residual(LevelGeom g, Coef<T> cf, const T* __restrict__ u, const T* __restrict__ f,
                            const T* __restrict__ k, T* __restrict__ r, double* __restrict__ partial) {
+    pdl_start();
     int x = blockIdx.x * blockDim.x + threadIdx.x;
     int y = blockIdx.y * blockDim.y + threadIdx.y;
     int z = blockIdx.z;
@@ -132,6 +141,7 @@ __global__ void k_residual(LevelGeom g, Coef<T> cf, const T* __restrict__ u, con
 // One block of 256 threads.  The order is fixed, so norms are reproducible run to run.
 __global__ void k_norm_finish(const double* __restrict__ partial, int n, double* __restrict__ hist,
                               int* __restrict__ slot, int cap, int advance, double* __restrict__ scalar_out) {
+    pdl_start();
     double s = 0.0;
     for (int i = threadIdx.x; i < n; i += blockDim.x) s += partial[i];
     double t = block_sum(s);
@@ -149,6 +159,7 @@ __global__ void k_norm_finish(const double* __restrict__ partial, int n, double*
 // coarse boundary entries 0.  Grid over the COARSE level.
 template <class T, int ND>
 __global__ void k_restrict(LevelGeom gc, LevelGeom gf, const T* __restrict__ fine, T* __restrict__ coarse) {
+    pdl_start();
     HOMG_NODE_XYZ(gc);
     long long cc = lidx(gc, x, y, z);
     if (!is_interior<ND>(gc, x, y, z)) { coarse[cc] = T(0); return; }
@@ -203,6 +214,7 @@ __device__ __forceinline__ T node_interp(const LevelGeom& gc, const T* __restric
 template <class T, int ND>
 __global__ void k_deliver(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, const T* __restrict__ ac,
                           T* __restrict__ ef, T* __restrict__ af, int ef_assign, int af_mode) {
+    pdl_start();
     HOMG_NODE_XYZ(gf);
     long long c = lidx(gf, x, y, z);
     T inc = ac ? node_interp<T, ND>(gc, ac, nullptr, x, y, z) : T(0);
@@ -216,6 +228,7 @@ __global__ void k_deliver(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, 
 // inject level m-1 -> m: e_c(P) = e_f(2P).  Grid over the COARSE level.   (one array)
 template <class T, int ND>
 __global__ void k_inject(LevelGeom gc, LevelGeom gf, const T* __restrict__ ef, T* __restrict__ ec) {
+    pdl_start();
     HOMG_NODE_XYZ(gc);
     ec[lidx(gc, x, y, z)] = ef[lidx(gf, 2 * x, 2 * y, ND == 3 ? 2 * z : 0)];
 }
@@ -225,6 +238,7 @@ __global__ void k_inject(LevelGeom gc, LevelGeom gf, const T* __restrict__ ef, T
 template <class T, int ND>
 __global__ void k_d0_up(LevelGeom gt, LevelGeom gv, int s, const T* __restrict__ X, const T* __restrict__ Y,
                         T* __restrict__ d0) {
+    pdl_start();
     HOMG_NODE_XYZ(gt);
     long long q = lidx(gv, x * s, y * s, ND == 3 ? z * s : 0);
     d0[lidx(gt, x, y, z)] = X[q] - Y[q];
@@ -237,6 +251,7 @@ template <class T, int ND>
 __global__ void k_d0_down(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, const T* __restrict__ B,
                           T* __restrict__ out, int coin_s, LevelGeom gv, const T* __restrict__ X,
                           const T* __restrict__ Y) {
+    pdl_start();
     HOMG_NODE_XYZ(gf);
     T val;
     bool coin = coin_s > 0 && (x % coin_s == 0) && (y % coin_s == 0) && (ND == 2 || (z % coin_s == 0));
@@ -258,6 +273,7 @@ template <class T, int ND, bool VAR>
 __global__ void k_relax(LevelGeom g, Coef<T> cf, const T* __restrict__ vin, const T* __restrict__ gsrc,
                         const T* __restrict__ k, T* __restrict__ vout, T* __restrict__ a, int a_assign,
                         const T* __restrict__ d0, const T* __restrict__ v0, T* __restrict__ u) {
+    pdl_start();
     HOMG_NODE_XYZ(g);
     long long c = lidx(g, x, y, z);
     if (!is_interior<ND>(g, x, y, z)) {
@@ -277,6 +293,7 @@ __global__ void k_relax(LevelGeom g, Coef<T> cf, const T* __restrict__ vin, cons
 // dense user array (C order, nx contiguous) <-> padded level-0 array.  to_padded: boundary -> 0.
 template <class T, int ND>
 __global__ void k_pack(LevelGeom g, const T* __restrict__ dense, T* __restrict__ padded, int zero_boundary) {
+    pdl_start();
     HOMG_NODE_XYZ(g);
     long long d = ((long long)z * g.ny + y) * g.nx + x;
     T v = dense[d];
@@ -286,6 +303,7 @@ __global__ void k_pack(LevelGeom g, const T* __restrict__ dense, T* __restrict__
 
 template <class T, int ND>
 __global__ void k_unpack(LevelGeom g, const T* __restrict__ padded, T* __restrict__ dense) {
+    pdl_start();
     HOMG_NODE_XYZ(g);
     dense[((long long)z * g.ny + y) * g.nx + x] = padded[lidx(g, x, y, z)];
 }
@@ -294,6 +312,7 @@ __global__ void k_unpack(LevelGeom g, const T* __restrict__ padded, T* __restric
 // (same kernel as k_inject; kept under its own name for the profile listing)
 template <class T, int ND>
 __global__ void k_sample_coef(LevelGeom gc, LevelGeom gf, const T* __restrict__ kf, T* __restrict__ kc) {
+    pdl_start();
     HOMG_NODE_XYZ(gc);
     kc[lidx(gc, x, y, z)] = kf[lidx(gf, 2 * x, 2 * y, ND == 3 ? 2 * z : 0)];
 }
