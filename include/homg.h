@@ -153,7 +153,7 @@ enum {
     HOMG_TAG_RESIDUAL0 = 0, /* level-0 residual (+norm partials, + first restriction when fused) */
     HOMG_TAG_NORM_FINISH,   /* fixed-order sum of the partials                                    */
     HOMG_TAG_RESTRICT,      /* full weighting g_m = P g_{m-1}                                     */
-    HOMG_TAG_RELAX0,        /* level-0 Jacobi sweeps (incl. fused interpolate+correct, u += e)    */
+    HOMG_TAG_RELAX0,        /* level-0 plain Jacobi sweeps                                        */
     HOMG_TAG_RELAX,         /* Jacobi sweeps on levels >= 1                                       */
     HOMG_TAG_DELIVER0,      /* interpolate+correct onto level 0 when not fused into the sweep     */
     HOMG_TAG_DELIVER,       /* interpolate+correct onto levels >= 1                               */
@@ -161,6 +161,8 @@ enum {
     HOMG_TAG_D0,            /* carried variation                                                  */
     HOMG_TAG_COARSE,        /* the persistent coarse-level launch                                 */
     HOMG_TAG_OTHER,
+    HOMG_TAG_RELAX0_FIRST,  /* level-0 first sweep with interpolate+correct fused (K_relax, first)        */
+    HOMG_TAG_RELAX0_LAST,   /* level-0 last sweep of the cycle with u += e fused                          */
     HOMG_TAG_COUNT
 };
 HOMG_API homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* launches_by_tag,

@@ -263,7 +263,8 @@ homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* l
 
 const char* homg_tag_name(int tag) {
     static const char* names[HOMG_TAG_COUNT] = {"residual_l0", "norm_finish", "restrict", "relax_l0", "relax_coarse",
-                                                "deliver_l0", "deliver", "inject", "d0", "coarse_persistent", "other"};
+                                                "deliver_l0", "deliver", "inject", "d0", "coarse_persistent", "other",
+                                                "relax_l0_first", "relax_l0_last"};
     return (tag >= 0 && tag < HOMG_TAG_COUNT) ? names[tag] : "";
 }
 

@@ -460,7 +460,7 @@ void rec_cycle(Rec& R) {
             bool last = (it == eta - 1);
             bool book = last && t >= 1;
             bool addu = last && vi == nv - 1;
-            const int tag = small(t) ? TAG_COARSE : (t == 0 ? TAG_RELAX0 : TAG_RELAX);
+            const int tag = small(t) ? TAG_COARSE : (t != 0 ? TAG_RELAX : (fuse_first && it == 0) ? TAG_RELAX0_FIRST : addu ? TAG_RELAX0_LAST : TAG_RELAX0);
             if (fuse_first && it == 0) {
                 flush();
                 if (!R.plan) launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
