@@ -163,6 +163,8 @@ enum {
     HOMG_TAG_OTHER,
     HOMG_TAG_RELAX0_FIRST,  /* level-0 first sweep with interpolate+correct fused (K_relax, first)        */
     HOMG_TAG_RELAX0_LAST,   /* level-0 last sweep of the cycle with u += e fused                          */
+    HOMG_TAG_VISIT0,        /* K_visit on level 0: interpolate+correct + all sweeps of the visit + u += e  */
+    HOMG_TAG_VISIT,         /* K_visit on levels >= 1: all sweeps of a visit + S3e bookkeeping            */
     HOMG_TAG_COUNT
 };
 HOMG_API homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* launches_by_tag,

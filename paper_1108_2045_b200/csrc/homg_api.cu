@@ -108,6 +108,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (const char* ev = std::getenv("HOMG_MARCH_CHUNK")) s->march_chunk = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_PDL")) s->pdl = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
+    if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);
     s->hist_cap = hist_cap;
     if (build_schedule(o.schedule, levels, s->max_iters, o.sched_levels, o.sched_iters, o.sched_len, s->sched_lv,
@@ -264,7 +265,7 @@ homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* l
 const char* homg_tag_name(int tag) {
     static const char* names[HOMG_TAG_COUNT] = {"residual_l0", "norm_finish", "restrict", "relax_l0", "relax_coarse",
                                                 "deliver_l0", "deliver", "inject", "d0", "coarse_persistent", "other",
-                                                "relax_l0_first", "relax_l0_last"};
+                                                "relax_l0_first", "relax_l0_last", "visit_l0", "visit"};
     return (tag >= 0 && tag < HOMG_TAG_COUNT) ? names[tag] : "";
 }
 

@@ -11,6 +11,7 @@
 
 #include "homg_coarse.cuh"
 #include "homg_first.cuh"
+#include "homg_visit.cuh"
 
 namespace homg {
 
@@ -169,6 +170,7 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
         int nch = 1;
         int mc = march_chunk<T, ND>(s, Lt.g, &nch);
         dim3 grid((Lt.g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (Lt.g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
+        if (u && t == 0) vout = nullptr;              // e_0 is dead after u += e_0: do not write it
         klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
                                                                                       d0, v0, u, mc);
     } else {
@@ -206,7 +208,54 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
     int nch = (interior + mc - 1) / mc;
     dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
     klaunch(R, k_relax_first<T, ND, VAR>, grid, TL::NW * 32, first_smem_bytes<T, ND, VAR>(), 
-        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), vout, u, mc);
+        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), (u && t == 0) ? (T*)nullptr : vout, u, mc);
+}
+
+
+// K_visit: NS sweeps of a visit on a large 3-D level in one pass (homg_visit.cuh).
+//   interp: stage 0 built from (ec, ac) of level t+1;  otherwise stage 0 = `in` (level t)
+template <class T, int NS, bool INTERP>
+void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
+                   const T* d0, const T* v0, T* u) {
+    homg_solver* s = R.s;
+    Level& Lt = s->L[t];
+    using TL = VisitTile<T, NS>;
+    CUtensorMap tm_in, tm_ac, tm_g;
+    bool ok = make_tmap<T, 3>(s, &tm_g, Lt.gsrc, Lt.g, TL::TXN, TL::PY);
+    if (INTERP) {
+        Level& Lc = s->L[t + 1];
+        ok = ok && make_tmap<T, 3>(s, &tm_in, ec, Lc.g, TL::CW, TL::CR) && make_tmap<T, 3>(s, &tm_ac, ac, Lc.g, TL::CW, TL::CR);
+    } else {
+        ok = ok && make_tmap<T, 3>(s, &tm_in, in, Lt.g, TL::TXN, TL::PY);
+        tm_ac = tm_in;
+    }
+    if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
+    const LevelGeom& g = Lt.g;
+    const int interior = std::max(g.nz - 2, 1);
+    const int tx = (g.nx - 1 + TL::OX - 1) / TL::OX, ty = (g.ny - 1 + TL::OY - 1) / TL::OY;
+    const long long tiles = (long long)tx * ty;
+    // z chunks: one CTA per SM; pick the count that minimises waves x (planes per chunk + pipeline fill)
+    int best = 1;
+    double bestc = 1e300;
+    for (int nch = 1; nch <= 64 && nch <= interior; ++nch) {
+        const int mc = (interior + nch - 1) / nch;
+        const long long waves = (tiles * nch + s->sm_count - 1) / s->sm_count;
+        const double c = double(waves) * double(mc + 2 * NS + 6);
+        if (c < bestc) { bestc = c; best = nch; }
+    }
+    int mc = s->march_chunk > 0 ? std::min(s->march_chunk, interior) : (interior + best - 1) / best;
+    const int nch = (interior + mc - 1) / mc;
+    dim3 grid(tx, ty, nch);
+    klaunch(R, k_visit3<T, NS, INTERP>, grid, TL::NT, visit_smem_bytes<T, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
+            make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+}
+
+template <class T, bool INTERP>
+void launch_visit3_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
+                      int a_assign, const T* d0, const T* v0, T* u) {
+    if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+    else if (ns == 3) launch_visit3<T, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+    else launch_visit3<T, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
 }
 
 
@@ -449,6 +498,60 @@ void rec_cycle(Rec& R) {
             }
             have_d0 = true;
         }
+        // K_visit: the whole visit (or, on level 0, chunks of up to 4 sweeps) in one pass over HBM
+        const int maxns = std::min(s->fuse_visit, 4);
+        if (ND == 3 && !VAR && maxns >= 2 && tiled(s, t) && !small(t) && eta >= 2 && (t == 0 || eta <= maxns)) {
+            flush();
+            const int v0i = Lt.e;
+            int in = v0i, i1 = -1, i2 = -1, done = 0;           // rot indices of v^k, v^{k-1}, v^{k-2}
+            bool interp = fuse_first;
+            while (done < eta) {
+                const int rem = eta - done;
+                const int ns = rem >= maxns ? maxns : rem;
+                const bool lastc = done + ns == eta;
+                const bool addu = lastc && vi == nv - 1 && t == 0;
+                const bool book = lastc && t >= 1;
+                if (ns == 1) {                                   // a single trailing sweep (level 0 only)
+                    int out = -1;
+                    for (int b = 0; b < Lt.nrot; ++b) if (b != in) { out = b; break; }
+                    if (!R.plan) launch_relax<T, ND, VAR>(R, t, rotp<T>(Lt, in), rotp<T>(Lt, out), nullptr, 0, nullptr, nullptr, addu ? (T*)s->u : nullptr);
+                    R.check(addu ? TAG_RELAX0_LAST : TAG_RELAX0);
+                    R.acct(t, 3.0 + (addu ? 1.0 : 0.0));
+                    i2 = i1; i1 = in; in = out; done += 1;
+                    continue;
+                }
+                int ob[3] = {-1, -1, -1}, nb = 0;               // free buffers: not the input, not v^0 (t >= 1)
+                for (int b = 0; b < Lt.nrot && nb < 3; ++b)
+                    if (b != in && !(t >= 1 && b == v0i)) ob[nb++] = b;
+                const int b0 = ob[0], b1 = t >= 1 ? ob[1] : -1, b2 = (t >= 1 && ns >= 3) ? ob[2] : -1;
+                T* o0 = addu ? nullptr : rotp<T>(Lt, b0);
+                const int tag = t == 0 ? TAG_VISIT0 : TAG_VISIT;
+                if (!R.plan) {
+                    if (interp)
+                        launch_visit3_ns<T, true>(R, ns, t, nullptr, fuse_ec, (const T*)L[t + 1].a, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                                                  nullptr, 0, nullptr, nullptr, addu ? (T*)s->u : nullptr);
+                    else
+                        launch_visit3_ns<T, false>(R, ns, t, rotp<T>(Lt, in), nullptr, nullptr, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                                                   book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, (book && have_d0) ? (const T*)Lt.d0 : nullptr,
+                                                   rotp<T>(Lt, v0i), addu ? (T*)s->u : nullptr);
+                }
+                R.check(tag);
+                if (interp) R.acct(t + 1, 2.0, tag);
+                R.acct(t, (interp ? 0.0 : 1.0) + 1.0 + (o0 ? 1.0 : 0.0) + (b1 >= 0 ? 1.0 : 0.0) + (b2 >= 0 ? 1.0 : 0.0) +
+                              (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) : 0.0) + (addu ? 2.0 : 0.0), tag);
+                // rot indices of the last three iterates
+                if (ns >= 3) { i2 = b2; i1 = b1; }
+                else { i2 = in; i1 = b1; }                        // ns == 2: v^{k-2} is this chunk's input
+                in = b0;
+                interp = false;
+                done += ns;
+            }
+            if (t >= 1) a_zero[t] = 0;
+            Lt.vk = in; Lt.vkm1 = i1; Lt.vkm2 = i2; Lt.e = in; Lt.eta_last = eta;
+            dp_is_d0[t] = false;
+            cur = t;
+            continue;
+        }
         // S3d eta damped-Jacobi sweeps; S3e bookkeeping fused into the last one; S4 u += e fused
         // into the last sweep of the cycle.
         const int v0 = Lt.e;
@@ -466,7 +569,7 @@ void rec_cycle(Rec& R) {
                 if (!R.plan) launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
                 R.check(tag);
                 R.acct(t + 1, 2.0, tag);
-                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 2.0 : 0.0), tag);
+                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 1.0 : 0.0), tag);
                 prev2 = prev_in; prev_in = in; in = out;
                 continue;
             }
@@ -486,7 +589,7 @@ void rec_cycle(Rec& R) {
                 R.check(tag);
             }
             R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
-                          (addu ? 2.0 : 0.0), tag);
+                          (addu ? (tiled(s, t) && t == 0 ? 1.0 : 2.0) : 0.0), tag);
             prev2 = prev_in; prev_in = in; in = out;
         }
         if (t >= 1) a_zero[t] = 0;
@@ -557,6 +660,15 @@ cudaError_t set_attr() {
                                 res_smem_bytes<T, ND, VAR>());
 }
 
+template <class T, int NS>
+cudaError_t set_attr_visit() {
+    cudaError_t e = cudaFuncSetAttribute(k_visit3<T, NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         visit_smem_bytes<T, NS, false>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_visit3<T, NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                visit_smem_bytes<T, NS, true>());
+}
+
 }  // namespace
 
 cudaError_t exec_init(homg_solver* s) {
@@ -576,6 +688,12 @@ cudaError_t exec_init(homg_solver* s) {
     if ((e = set_attr<double, 2, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, true>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<float, 2>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<float, 3>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<float, 4>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<double, 2>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<double, 3>()) != cudaSuccess) return e;
+    if ((e = set_attr_visit<double, 4>()) != cudaSuccess) return e;
     return cudaSuccess;
 }
 

@@ -7,7 +7,7 @@ namespace homg {
 // kernel classes reported by homg_profile_cycles (order = include/homg.h HOMG_TAG_*)
 enum {
     TAG_RESIDUAL0 = 0, TAG_NORM_FINISH, TAG_RESTRICT, TAG_RELAX0, TAG_RELAX, TAG_DELIVER0, TAG_DELIVER,
-    TAG_INJECT, TAG_D0, TAG_COARSE, TAG_OTHER, TAG_RELAX0_FIRST, TAG_RELAX0_LAST, TAG_COUNT
+    TAG_INJECT, TAG_D0, TAG_COARSE, TAG_OTHER, TAG_RELAX0_FIRST, TAG_RELAX0_LAST, TAG_VISIT0, TAG_VISIT, TAG_COUNT
 };
 
 constexpr long long kTiledMinNodesDefault = 200000;   // 65^3 and up, 449^2 and up

@@ -281,7 +281,7 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
                 out.v[j] = xin[j] ? vc + (VAR ? num / D : div_const(num, cf.D, cf.rD)) : T(0);
             }
             if (owned) {
-                *reinterpret_cast<Pack<T>*>(vout + c) = out;
+                if (vout) *reinterpret_cast<Pack<T>*>(vout + c) = out;
                 if (u) {
                     Pack<T> uu = *reinterpret_cast<const Pack<T>*>(u + c);
 #pragma unroll

@@ -73,6 +73,7 @@ __host__ __device__ constexpr int relax_smem_bytes() {
 // S3d (+S3e, +S4): one damped-Jacobi sweep  vout = vin + w (g - A vin)/D  on a large level.
 //   tmv / tmk / tmg : tensor maps of vin, k (VAR) and g of this level
 //   a, a_assign, d0, v0, u : the optional epilogues of k_relax (same meaning)
+//   vout may be null when u is given (last sweep of the cycle: e_0 is dead after u += e_0)
 //   mchunk : interior planes per CTA along the marching axis
 // grid = (x tiles, y tiles, chunks) in 3-D, (x tiles, chunks) in 2-D.      (Eq.2-3)
 template <class T, int ND, bool VAR>
@@ -207,7 +208,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
             out.v[j] = xin[j] ? vc + (VAR ? num / D : div_const(num, cf.D, cf.rD)) : T(0);
         }
         if (row_ok) {
-            *reinterpret_cast<Pack<T>*>(vout + c) = out;
+            if (vout) *reinterpret_cast<Pack<T>*>(vout + c) = out;
             if (a) {
                 Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(v0 + c), aa;
                 if (d0) dd = *reinterpret_cast<const Pack<T>*>(d0 + c);

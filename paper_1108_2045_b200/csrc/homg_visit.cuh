@@ -1,0 +1,298 @@
+// homg_visit.cuh — K_visit: one whole MFMG visit of a large 3-D level in ONE pass over HBM
+// (north_star item 2, taken one step further: interpolate + correct + NS Jacobi sweeps [+ u += e]).
+//
+// A visit is NS damped-Jacobi sweeps v^s = v^{s-1} + w D^-1 (g - A v^{s-1}), s = 1..NS (PAPER.md
+// L53-67, Eq. 2-3), on the same level.  Run as NS launches it moves 3 arrays per sweep.  Here a CTA
+// owns an x/y tile, marches along z and keeps a software pipeline of the NS sweeps in flight:
+// at step q the plane z0 = zs+q of v^0 arrives, and stage s computes plane z0-s of v^s from the
+// planes z0-s-1, z0-s, z0-s+1 of v^{s-1}.  Every thread owns one 16-byte pack of x nodes of one row
+// and carries its own column of every v^{s-1} (previous / current / next plane) in registers; the
+// in-plane neighbours come from shared memory (y) and warp shuffles (x).  Each stage publishes the
+// plane it produced in a 2-slot shared-memory buffer for the next stage's y neighbours, so one
+// __syncthreads per step suffices.  The tile carries a halo of NS nodes per side that is
+// recomputed (valid region shrinks by one node per stage); only the inner OX x OY nodes are stored.
+//
+// HBM traffic of a level-0 visit (NS = 4): read g, read the two coarse arrays (INTERP) or v^0,
+// read+write u  =  (3 + 2/8) passes instead of (2 + 2/8) + 3 + 3 + 4.
+//
+// Stage 0 is either PLAIN (v^0 planes staged by TMA) or INTERP (S3a: v^0 built in shared memory
+// from the coarse planes of e_c and a_c, as in homg_first.cuh).  Epilogues of the last stage are
+// those of k_relax: S3e bookkeeping (a += d0 + v^{NS-1} - v^0) and S4 (u += v^NS); the last three
+// iterates can be stored (o0 = v^NS, o1 = v^{NS-1}, o2 = v^{NS-2}) because the next visit's carried
+// variation needs them (S3c).
+//
+// The arithmetic per node is the expression tree of homg_kernels.cuh (R14): results are
+// bit-identical to NS launches of the single-sweep kernels and to the oracle.
+#pragma once
+#include "homg_fused.cuh"
+
+namespace homg {
+
+template <class T, int NS>
+struct VisitTile {
+    static constexpr int ES = int(sizeof(T));
+    static constexpr int VEC = 16 / ES;
+    static constexpr int PX = 16, PY = 32, NT = PX * PY;      // packs per row, rows, threads
+    static constexpr int HX = (NS + VEC - 1) / VEC * VEC;     // x halo (nodes), pack granular
+    static constexpr int HY = NS;
+    static constexpr int TXN = PX * VEC;                      // tile width in nodes
+    static constexpr int OX = TXN - 2 * HX, OY = PY - 2 * HY; // nodes stored per plane
+    static constexpr int RS = TXN;                            // row stride (elements) = 256 B
+    static constexpr int PLANE = (PY + 2) * RS;               // one pad row below and one above
+    static constexpr int PLANE_BYTES = PLANE * ES;
+    static constexpr int BOX_BYTES = PY * RS * ES;            // one TMA box {TXN, PY, 1}
+    static constexpr int NIN = 4;                             // TMA ring depth of the v^0 planes
+    static constexpr int NGR = 8;                             // g ring: plane z0-s is read by stage s (NS <= 4)
+    // coarse tiles of e_c and a_c (INTERP)
+    static constexpr int CWN = TXN / 2 + 1;                   // coarse columns a tile row needs
+    static constexpr int CW = (CWN + 2 * (VEC - 1)) / VEC * VEC;   // + slack: the box starts 16-B aligned
+    static constexpr int CR = PY / 2 + 2;
+    static constexpr int CBOX_BYTES = CR * CW * ES;
+    static constexpr int CTILE_BYTES = (CBOX_BYTES + 127) / 128 * 128;
+    static constexpr int NC = 4;
+};
+
+template <class T, int NS, bool INTERP>
+__host__ __device__ constexpr int visit_smem_bytes() {
+    using TL = VisitTile<T, NS>;
+    return TL::NGR * TL::BOX_BYTES +
+           (INTERP ? TL::NC * 2 * TL::CTILE_BYTES + NS * 2 * TL::PLANE_BYTES
+                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + 128;
+}
+
+// tm_in : PLAIN: v^0 of this level, box {TXN, PY, 1};  INTERP: e_c of level c = t+1, box {CW, CR, 1}
+// tm_ac : INTERP: a_c, same box;  tm_g : g of this level, box {TXN, PY, 1}
+// o0 / o1 / o2 : v^NS, v^{NS-1}, v^{NS-2} (each may be null);  a, a_assign, d0, v0, u : as k_relax
+// grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior planes)
+template <class T, int NS, bool INTERP>
+__global__ void __launch_bounds__(VisitTile<T, NS>::NT, 1)
+k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
+         const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
+         T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
+         const T* __restrict__ v0, T* __restrict__ u, int mchunk) {
+    pdl_start();
+    using TL = VisitTile<T, NS>;
+    constexpr int VEC = TL::VEC, RS = TL::RS;
+    const int tid = threadIdx.x, px = tid % TL::PX, py = tid / TL::PX;
+    const int x0 = blockIdx.x * TL::OX, y0 = blockIdx.y * TL::OY;
+    const int ms = 1 + blockIdx.z * mchunk;
+    const int me = min(ms + mchunk, g.nz - 1);
+    if (ms >= me) return;
+    const int zs = ms - NS;                                        // first plane of stage 0
+    const int nsteps = me - ms + 2 * NS;                           // one stage-0 plane per step
+    const int Zc0 = zs >> 1;                                       // first coarse plane (floor)
+    const int ncz = ((me + NS) >> 1) - Zc0 + 1;
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+    __shared__ uint64_t fbar[TL::NIN], gbar[TL::NGR], cbar[TL::NC];
+    auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * TL::BOX_BYTES); };
+    unsigned char* cbase = smem + TL::NGR * TL::BOX_BYTES;         // PLAIN: v ring;  INTERP: coarse ring
+    auto vring = [&](int st) { return reinterpret_cast<T*>(cbase + st * TL::PLANE_BYTES); };
+    auto ce = [&](int st) { return reinterpret_cast<T*>(cbase + (2 * st) * TL::CTILE_BYTES); };
+    auto ca = [&](int st) { return reinterpret_cast<T*>(cbase + (2 * st + 1) * TL::CTILE_BYTES); };
+    unsigned char* sbase = cbase + (INTERP ? TL::NC * 2 * TL::CTILE_BYTES : TL::NIN * TL::PLANE_BYTES);
+    auto buf = [&](int s, int slot) {                              // plane published by stage s
+        return reinterpret_cast<T*>(sbase + ((INTERP ? s : s - 1) * 2 + slot) * TL::PLANE_BYTES);
+    };
+
+    if (tid == 0) {
+        for (int s = 0; s < TL::NIN; ++s) mbar_init(&fbar[s], 1);
+        for (int s = 0; s < TL::NGR; ++s) mbar_init(&gbar[s], 1);
+        for (int s = 0; s < TL::NC; ++s) mbar_init(&cbar[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int Xc = (x0 - TL::HX) / 2;                              // x0 - HX is even
+    const int Xa = Xc - (Xc & (VEC - 1));                          // coarse box start, 16-B aligned
+    const int Yc = (y0 - TL::HY) >> 1;
+    auto issue_f = [&](int q) {                                    // fine plane zs+q: (v^0 and) g
+        const int st = q & (TL::NIN - 1), sg = q & (TL::NGR - 1), p = zs + q;
+        if (!INTERP) {
+            mbar_arrive_expect_tx(&fbar[st], TL::BOX_BYTES);
+            tma_load_3d(vring(st) + RS, &tm_in, &fbar[st], x0 - TL::HX, y0 - TL::HY, p);
+        }
+        mbar_arrive_expect_tx(&gbar[sg], TL::BOX_BYTES);
+        tma_load_3d(gs(sg), &tm_g, &gbar[sg], x0 - TL::HX, y0 - TL::HY, p);
+    };
+    auto issue_c = [&](int zc) {                                   // coarse plane Zc0+zc of e_c and a_c
+        const int st = zc & (TL::NC - 1);
+        mbar_arrive_expect_tx(&cbar[st], 2 * TL::CBOX_BYTES);
+        tma_load_3d(ce(st), &tm_in, &cbar[st], Xa, Yc, Zc0 + zc);
+        tma_load_3d(ca(st), &tm_ac, &cbar[st], Xa, Yc, Zc0 + zc);
+    };
+    if (tid == 0) {
+        if (INTERP)
+            for (int zc = 0; zc < TL::NC && zc < ncz; ++zc) issue_c(zc);
+        for (int q = 0; q < TL::NIN - 1 && q < nsteps; ++q) issue_f(q);
+    }
+
+    // ---- this thread's pack: nodes x .. x+VEC-1 of row y ----
+    const int x = x0 - TL::HX + px * VEC;
+    const int y = y0 - TL::HY + py;
+    const int off = (py + 1) * RS + px * VEC;                      // in a padded plane
+    const int goff = py * RS + px * VEC;
+    const bool row_int = y > 0 && y < g.ny - 1;
+    bool xin[VEC];
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) xin[j] = row_int && (x + j > 0) && (x + j < g.nx - 1);
+    const bool own = px * VEC >= TL::HX && px * VEC < TL::HX + TL::OX && x < g.nx && py >= TL::HY &&
+                     py < TL::HY + TL::OY && y < g.ny;
+    // INTERP: my first coarse node inside a coarse tile
+    const int yl = (y >> 1) - Yc;
+    const bool yodd = y & 1;
+    const int coff = yl * TL::CW + (Xc - Xa) + px * (VEC / 2);
+
+    // S3a in registers: the pack of v^0 at fine plane z from the coarse planes z>>1 and (z+1)>>1;
+    // summation order as homg_first.cuh / the oracle: rows (z lo, y lo), (z lo, y hi), (z hi, y lo), (z hi, y hi)
+    auto produce = [&](const int z) -> Pack<T> {
+        constexpr int NCV = VEC / 2 + 1;
+        const bool zodd = z & 1;
+        const int zlo = (z >> 1) - Zc0, zhi = ((z + 1) >> 1) - Zc0;
+        mbar_wait(&cbar[zlo & (TL::NC - 1)], (zlo / TL::NC) & 1);
+        if (zodd) mbar_wait(&cbar[zhi & (TL::NC - 1)], (zhi / TL::NC) & 1);
+        const T* A0 = ca(zlo & (TL::NC - 1)) + coff;
+        const T* A1 = ca(zhi & (TL::NC - 1)) + coff;
+        const T* E0 = ce(zlo & (TL::NC - 1)) + coff;
+        T acc[VEC];
+        auto addrow = [&](const T* rp, const bool first) {
+            T c[NCV];
+            if (VEC == 4) {
+                const HalfPack<T> h = *reinterpret_cast<const HalfPack<T>*>(rp);
+                c[0] = h.v[0]; c[1] = h.v[1]; c[NCV - 1] = rp[NCV - 1];
+            } else {
+#pragma unroll
+                for (int i = 0; i < NCV; ++i) c[i] = rp[i];
+            }
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) {
+                if (j & 1) { acc[j] = first ? c[j >> 1] : acc[j] + c[j >> 1]; acc[j] += c[(j >> 1) + 1]; }
+                else acc[j] = first ? c[j >> 1] : acc[j] + c[j >> 1];
+            }
+        };
+        addrow(A0, true);
+        if (yodd) addrow(A0 + TL::CW, false);
+        if (zodd) {
+            addrow(A1, false);
+            if (yodd) addrow(A1 + TL::CW, false);
+        }
+        const T wzy = (zodd && yodd) ? T(0.25) : ((zodd || yodd) ? T(0.5) : T(1));
+        const bool coin = !zodd && !yodd;
+        Pack<T> out;
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) {
+            if (j & 1) out.v[j] = (T(0.5) * wzy) * acc[j];
+            else out.v[j] = coin ? E0[j >> 1] : wzy * acc[j];
+        }
+        return out;
+    };
+
+    // register state: own column of every stage input (previous and current plane), g of the stages
+    Pack<T> P[NS], C[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) { P[s].v[j] = T(0); C[s].v[j] = T(0); }
+
+    // address of (x, y) in the plane the LAST stage produces at step q: z = zs + q - NS
+    long long cF = (long long)(zs - NS) * g.pp + (long long)y * g.px + x;
+
+    auto step = [&](auto KC, const int q) {
+        constexpr int K = decltype(KC)::value;                     // q mod 4
+        constexpr int W = K & 1, R = W ^ 1;                        // stage-buffer slots: written now / read now
+        constexpr int SC = (K + 3) & 3;                            // ring slot of plane z0-1
+        const int z0 = zs + q;
+        // ---- stage 0: the pack of v^0 at plane z0 ----
+        Pack<T> nx;
+        if (INTERP) {
+            nx = produce(z0);
+            *reinterpret_cast<Pack<T>*>(buf(0, W) + off) = nx;
+        } else {
+            mbar_wait(&fbar[K], (q / TL::NIN) & 1);
+            nx = *reinterpret_cast<const Pack<T>*>(vring(K) + off);
+        }
+        // u of the plane the last stage produces in this step: loaded now, used after the NS stages,
+        // so that its HBM latency hides behind the arithmetic
+        const bool fin = own && q >= 2 * NS;
+        Pack<T> uu;
+        if (fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
+        // stage s reads g of plane z0-s from the g ring; plane z0-1 is new in this step
+        if (q >= 1) mbar_wait(&gbar[(q - 1) & (TL::NGR - 1)], ((q - 1) / TL::NGR) & 1);
+#pragma unroll
+        for (int s = 1; s <= NS; ++s) {
+            // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
+            const T* ctr = (s == 1 && !INTERP) ? vring(SC) : buf(s - 1, R);
+            const Pack<T> dn = *reinterpret_cast<const Pack<T>*>(ctr + off - RS);
+            const Pack<T> up = *reinterpret_cast<const Pack<T>*>(ctr + off + RS);
+            const Pack<T> cu = C[s - 1], pv = P[s - 1];
+            const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
+            const T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
+            const T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
+            const int z = z0 - s;
+            const bool zin = z > 0 && z < g.nz - 1;
+            Pack<T> out;
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) {
+                const T vc = cu.v[j];
+                const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
+                const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+                T sm = pv.v[j] + nx.v[j];
+                sm += dn.v[j] + up.v[j];
+                sm += xm + xp;
+                const T Av = (cf.twod * vc - sm) * cf.ih2;
+                const T num = cf.w * (gv.v[j] - Av);
+                out.v[j] = xin[j] ? vc + div_const(num, cf.D, cf.rD) : T(0);
+            }
+            if (!zin) {                                            // Dirichlet planes z = 0, nz-1 (and beyond)
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) out.v[j] = T(0);
+            }
+            if (s < NS) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
+            if (s == NS - 2 && s >= 1 && o2 != nullptr && own && q >= 2 * NS - 2 && q <= nsteps - 3)
+                *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * g.pp) = out;
+            if (s == NS - 1 && s >= 1 && o1 != nullptr && own && q >= 2 * NS - 1 && q <= nsteps - 2)
+                *reinterpret_cast<Pack<T>*>(o1 + cF + g.pp) = out;
+            if (s == NS && fin) {
+                if (o0) *reinterpret_cast<Pack<T>*>(o0 + cF) = out;
+                if (a) {                                           // S3e: a (+)= d0 + v^{NS-1} - v^0
+                    Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(v0 + cF), aa;
+                    if (d0) dd = *reinterpret_cast<const Pack<T>*>(d0 + cF);
+                    if (!a_assign) aa = *reinterpret_cast<const Pack<T>*>(a + cF);
+#pragma unroll
+                    for (int j = 0; j < VEC; ++j) {
+                        const T Dq = ((d0 ? dd.v[j] : T(0)) + cu.v[j]) - vv.v[j];
+                        aa.v[j] = a_assign ? Dq : aa.v[j] + Dq;
+                    }
+                    *reinterpret_cast<Pack<T>*>(a + cF) = aa;
+                }
+                if (u) {                                           // S4: u += v^NS
+#pragma unroll
+                    for (int j = 0; j < VEC; ++j) uu.v[j] += out.v[j];
+                    *reinterpret_cast<Pack<T>*>(u + cF) = uu;
+                }
+            }
+            P[s - 1] = cu; C[s - 1] = nx; nx = out;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            if (q + TL::NIN - 1 < nsteps) issue_f(q + TL::NIN - 1);
+            if (INTERP && (z0 & 1)) {                              // coarse plane z0>>1 is dead now
+                const int zc = (z0 >> 1) - Zc0 + TL::NC;
+                if (zc < ncz) issue_c(zc);
+            }
+        }
+        cF += g.pp;
+    };
+    for (int q = 0; q < nsteps; q += 4) {
+        step(std::integral_constant<int, 0>{}, q);
+        if (q + 1 >= nsteps) break;
+        step(std::integral_constant<int, 1>{}, q + 1);
+        if (q + 2 >= nsteps) break;
+        step(std::integral_constant<int, 2>{}, q + 2);
+        if (q + 3 >= nsteps) break;
+        step(std::integral_constant<int, 3>{}, q + 3);
+    }
+}
+
+}  // namespace homg
