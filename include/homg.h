@@ -170,6 +170,11 @@ enum {
 HOMG_API homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* launches_by_tag,
                                          double* bytes_by_tag, int cap);
 HOMG_API const char* homg_tag_name(int tag);
+/* COMPULSORY bytes of one cycle per kernel class (bytes_by_tag nullable, cap entries) and their sum
+ * (return value): what each launch itself has to move.  Equal to the algorithmic bytes for every
+ * single-operation kernel; smaller for K_visit, which performs several Jacobi sweeps (3 arrays each
+ * in the per-sweep count of SURVEY.md 8(d)) in one pass.  Valid after the first homg_cycle. */
+HOMG_API double homg_compulsory_bytes_per_cycle(const homg_solver* s, double* bytes_by_tag, int cap);
 
 HOMG_API void homg_destroy(homg_solver* s);
 

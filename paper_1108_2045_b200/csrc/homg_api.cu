@@ -286,6 +286,16 @@ double homg_bytes_per_cycle(const homg_solver* s, int level0_only) {
     return level0_only ? s->bytes_cycle_l0 : s->bytes_cycle_all;
 }
 
+double homg_compulsory_bytes_per_cycle(const homg_solver* s, double* bytes_by_tag, int cap) {
+    if (!s) return -1.0;
+    double tot = 0.0;
+    for (int t = 0; t < HOMG_TAG_COUNT; ++t) {
+        if (bytes_by_tag && t < cap) bytes_by_tag[t] = s->comp_by_tag[t];
+        tot += s->comp_by_tag[t];
+    }
+    return tot;
+}
+
 void homg_destroy(homg_solver* s) {
     if (!s) return;
     drop_graph(s);

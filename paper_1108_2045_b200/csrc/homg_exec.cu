@@ -12,6 +12,7 @@
 #include "homg_coarse.cuh"
 #include "homg_first.cuh"
 #include "homg_visit.cuh"
+#include "homg_moves.cuh"
 
 namespace homg {
 
@@ -28,7 +29,8 @@ struct Rec {                 // bookkeeping while recording
     std::vector<cudaEvent_t>* ev = nullptr;   // profile mode: one event after every launch
     std::vector<int>* ev_tag = nullptr;
     int last_tag = TAG_OTHER;
-    double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class
+    double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class (per sweep)
+    double comp_tag[TAG_COUNT] = {};          // compulsory bytes per kernel class (what the launch must move)
     bool plan = false;                        // planning pass: build the coarse program, launch nothing
     std::vector<unsigned char> prog;          // CoarseOp records of the whole cycle, in order
     int prog_nops = 0, run_begin = 0, run_len = 0;
@@ -44,6 +46,13 @@ struct Rec {                 // bookkeeping while recording
         if (nodes > run_maxnodes) run_maxnodes = nodes;
     }
     void acct(int level, double arrays, int tag) { last_tag = tag; acct(level, arrays); }
+    // a fused multi-sweep launch: `arrays` = the per-sweep (algorithmic) passes it stands for,
+    // `comp` = the passes the fused launch itself has to move
+    void acct2(int level, double arrays, double comp, int tag) {
+        last_tag = tag;
+        acct(level, arrays);
+        comp_tag[tag] += (comp - arrays) * double(s->L[level].n_nodes) * double(s->dtype);
+    }
     void check(int tag) {
         last_tag = tag;
         if (plan) return;
@@ -67,6 +76,7 @@ struct Rec {                 // bookkeeping while recording
         double b = arrays * double(s->L[level].n_nodes) * double(s->dtype);
         bytes_all += b;
         bytes_tag[last_tag] += b;
+        comp_tag[last_tag] += b;
         if (level == 0) bytes_l0 += b;
     }
 };
@@ -90,6 +100,11 @@ inline dim3 d3(int x) { return dim3(x, 1, 1); }
 
 inline dim3 blk() { return dim3(32, 8, 1); }
 inline dim3 grd(const LevelGeom& g) { return dim3((g.nx + 31) / 32, (g.ny + 7) / 8, g.nz); }
+template <class T>
+inline dim3 grdv(const LevelGeom& g) {           // one 16-byte pack of x nodes per thread (homg_moves.cuh)
+    const int w = 32 * (16 / int(sizeof(T)));
+    return dim3((g.nx + w - 1) / w, (g.ny + 7) / 8, g.nz);
+}
 
 template <class T>
 Coef<T> make_coef(const homg_solver* s, int m) {
@@ -416,7 +431,7 @@ void rec_cycle(Rec& R) {
                         R.push(o, Lf.n_nodes);
                     } else {
                         flush();
-                        if (!R.plan) klaunch(R, k_deliver<T, ND>, grd(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
+                        if (!R.plan) klaunch(R, k_deliver_v<T, ND>, grdv<T>(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
                                                                                     rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
                         R.check(tag);
                     }
@@ -475,8 +490,8 @@ void rec_cycle(Rec& R) {
                             R.push(o, L[m - 1].n_nodes);
                         } else {
                             flush();
-                            if (!R.plan) klaunch(R, k_d0_down<T, ND>, grd(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,
-                                                                                              last ? (1 << (cur - t)) : 0, Lv.g, X, Y);
+                            if (!R.plan) klaunch(R, k_d0_down_v<T, ND>, grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,
+                                                                                                last ? (1 << (cur - t)) : 0, last ? cur - t : 0, Lv.g, X, Y);
                             R.check(tag);
                         }
                         R.acct(m, B ? 2.0 : 1.0, tag); R.acct(m - 1, 1.0, tag);
@@ -537,8 +552,14 @@ void rec_cycle(Rec& R) {
                 }
                 R.check(tag);
                 if (interp) R.acct(t + 1, 2.0, tag);
-                R.acct(t, (interp ? 0.0 : 1.0) + 1.0 + (o0 ? 1.0 : 0.0) + (b1 >= 0 ? 1.0 : 0.0) + (b2 >= 0 ? 1.0 : 0.0) +
-                              (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) : 0.0) + (addu ? 2.0 : 0.0), tag);
+                {
+                    // compulsory passes of the fused launch vs the per-sweep figures of SURVEY 8(d)
+                    const double bk = book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) : 0.0;
+                    const double comp = (interp ? 0.0 : 1.0) + 1.0 + (o0 ? 1.0 : 0.0) + (b1 >= 0 ? 1.0 : 0.0) +
+                                        (b2 >= 0 ? 1.0 : 0.0) + bk + (addu ? 2.0 : 0.0);
+                    const double alg = (interp ? 2.0 : 3.0) + 3.0 * (ns - 1) + (addu ? 1.0 : 0.0) + bk + (book ? 1.0 : 0.0);
+                    R.acct2(t, alg, comp, tag);
+                }
                 // rot indices of the last three iterates
                 if (ns >= 3) { i2 = b2; i1 = b1; }
                 else { i2 = in; i1 = b1; }                        // ns == 2: v^{k-2} is this chunk's input
@@ -719,6 +740,7 @@ cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     s->launches_per_cycle = R.launches;
     s->bytes_cycle_all = R.bytes_all;
     s->bytes_cycle_l0 = R.bytes_l0;
+    for (int t = 0; t < TAG_COUNT; ++t) s->comp_by_tag[t] = R.comp_tag[t];
     return R.err;
 }
 

@@ -95,5 +95,6 @@ struct homg_solver {
     long cycles_issued = 0;
     int launches_per_cycle = 0;
     double bytes_cycle_all = 0, bytes_cycle_l0 = 0;
+    double comp_by_tag[32] = {};         // compulsory bytes of one cycle per kernel class
     std::string err;
 };

@@ -198,10 +198,11 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
     // address of (x, y) in the plane the LAST stage produces at step q: z = zs + q - NS
     long long cF = (long long)(zs - NS) * g.pp + (long long)y * g.px + x;
 
-    auto step = [&](auto KC, const int q) {
-        constexpr int K = decltype(KC)::value;                     // q mod 4
-        constexpr int W = K & 1, R = W ^ 1;                        // stage-buffer slots: written now / read now
-        constexpr int SC = (K + 3) & 3;                            // ring slot of plane z0-1
+    // STEADY: the pipeline is full and every stage's plane is interior — no range checks
+    auto step = [&](auto KC, auto SD, const int q) {
+        constexpr int W = decltype(KC)::value, R = W ^ 1;          // stage-buffer slots: written now / read now
+        constexpr bool STEADY = decltype(SD)::value;
+        const int K = q & (TL::NIN - 1), SC = (q - 1) & (TL::NIN - 1);   // v ring slots of planes z0, z0-1
         const int z0 = zs + q;
         // ---- stage 0: the pack of v^0 at plane z0 ----
         Pack<T> nx;
@@ -214,11 +215,11 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         }
         // u of the plane the last stage produces in this step: loaded now, used after the NS stages,
         // so that its HBM latency hides behind the arithmetic
-        const bool fin = own && q >= 2 * NS;
+        const bool fin = own && (STEADY || q >= 2 * NS);
         Pack<T> uu;
         if (fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
         // stage s reads g of plane z0-s from the g ring; plane z0-1 is new in this step
-        if (q >= 1) mbar_wait(&gbar[(q - 1) & (TL::NGR - 1)], ((q - 1) / TL::NGR) & 1);
+        if (STEADY || q >= 1) mbar_wait(&gbar[(q - 1) & (TL::NGR - 1)], ((q - 1) / TL::NGR) & 1);
 #pragma unroll
         for (int s = 1; s <= NS; ++s) {
             // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
@@ -230,7 +231,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             const T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
             const T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
             const int z = z0 - s;
-            const bool zin = z > 0 && z < g.nz - 1;
+            const bool zin = STEADY || (z > 0 && z < g.nz - 1);
             Pack<T> out;
 #pragma unroll
             for (int j = 0; j < VEC; ++j) {
@@ -249,9 +250,9 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 for (int j = 0; j < VEC; ++j) out.v[j] = T(0);
             }
             if (s < NS) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
-            if (s == NS - 2 && s >= 1 && o2 != nullptr && own && q >= 2 * NS - 2 && q <= nsteps - 3)
+            if (s == NS - 2 && s >= 1 && o2 != nullptr && own && (STEADY || (q >= 2 * NS - 2 && q <= nsteps - 3)))
                 *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * g.pp) = out;
-            if (s == NS - 1 && s >= 1 && o1 != nullptr && own && q >= 2 * NS - 1 && q <= nsteps - 2)
+            if (s == NS - 1 && s >= 1 && o1 != nullptr && own && (STEADY || (q >= 2 * NS - 1 && q <= nsteps - 2)))
                 *reinterpret_cast<Pack<T>*>(o1 + cF + g.pp) = out;
             if (s == NS && fin) {
                 if (o0) *reinterpret_cast<Pack<T>*>(o0 + cF) = out;
@@ -284,14 +285,18 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         }
         cF += g.pp;
     };
-    for (int q = 0; q < nsteps; q += 4) {
-        step(std::integral_constant<int, 0>{}, q);
-        if (q + 1 >= nsteps) break;
-        step(std::integral_constant<int, 1>{}, q + 1);
-        if (q + 2 >= nsteps) break;
-        step(std::integral_constant<int, 2>{}, q + 2);
-        if (q + 3 >= nsteps) break;
-        step(std::integral_constant<int, 3>{}, q + 3);
+    using I0 = std::integral_constant<int, 0>;
+    using I1 = std::integral_constant<int, 1>;
+    for (int q = 0; q < nsteps; q += 2) {
+        // steps q and q+1 are steady when all their stores are due and planes z0-NS .. z0-1 are interior
+        const bool steady = q >= 2 * NS && q + 1 <= nsteps - 3 && zs + q - NS >= 1 && zs + q <= g.nz - 2;
+        if (steady) {
+            step(I0{}, std::true_type{}, q);
+            step(I1{}, std::true_type{}, q + 1);
+        } else {
+            step(I0{}, std::false_type{}, q);
+            if (q + 1 < nsteps) step(I1{}, std::false_type{}, q + 1);
+        }
     }
 }
 

@@ -20,7 +20,7 @@ DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
 SYMBOLS = [
     "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
     "homg_set_coefficient", "homg_cycle", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
-    "homg_profile_cycles", "homg_tag_name", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
+    "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
 ]
 
 
@@ -67,6 +67,7 @@ def lib():
         L.homg_bytes_per_cycle.argtypes = [vp, i]; L.homg_bytes_per_cycle.restype = d
         L.homg_profile_cycles.argtypes = [vp, i, C.POINTER(d), C.POINTER(i), C.POINTER(d), i]; L.homg_profile_cycles.restype = i
         L.homg_tag_name.argtypes = [i]; L.homg_tag_name.restype = C.c_char_p
+        L.homg_compulsory_bytes_per_cycle.argtypes = [vp, C.POINTER(d), i]; L.homg_compulsory_bytes_per_cycle.restype = d
         L.homg_destroy.argtypes = [vp]; L.homg_destroy.restype = None
         L.homg_last_error.argtypes = [vp]; L.homg_last_error.restype = C.c_char_p
         _lib = L
@@ -186,6 +187,13 @@ class Solver:
 
     def bytes_per_cycle(self, level0_only=False):
         return float(lib().homg_bytes_per_cycle(self.handle, 1 if level0_only else 0))
+
+    def compulsory_bytes_per_cycle(self):
+        """{kernel class: bytes the launches of one cycle themselves must move}, and the total."""
+        cap = 32
+        by = (C.c_double * cap)()
+        tot = float(lib().homg_compulsory_bytes_per_cycle(self.handle, by, cap))
+        return {lib().homg_tag_name(t).decode(): by[t] for t in range(cap) if lib().homg_tag_name(t) and by[t]}, tot
 
     def profile_cycles(self, n=1):
         """{kernel class: (total ms, launches, algorithmic bytes)} over n real cycles with per-launch CUDA events."""
