@@ -227,52 +227,53 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
 }
 
 
-// K_visit: NS sweeps of a visit on a large 3-D level in one pass (homg_visit.cuh).
+// K_visit: NS sweeps of a visit on a large level in one pass (homg_visit.cuh).
 //   interp: stage 0 built from (ec, ac) of level t+1;  otherwise stage 0 = `in` (level t)
-template <class T, int NS, bool INTERP>
-void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
-                   const T* d0, const T* v0, T* u) {
+template <class T, int ND, int NS, bool INTERP>
+void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
+                  const T* d0, const T* v0, T* u) {
     homg_solver* s = R.s;
     Level& Lt = s->L[t];
-    using TL = VisitTile<T, NS>;
+    using TL = VisitTile<T, ND, NS>;
     CUtensorMap tm_in, tm_ac, tm_g;
-    bool ok = make_tmap<T, 3>(s, &tm_g, Lt.gsrc, Lt.g, TL::TXN, TL::PY);
+    bool ok = make_tmap<T, ND>(s, &tm_g, Lt.gsrc, Lt.g, TL::BW, TL::PY);
     if (INTERP) {
         Level& Lc = s->L[t + 1];
-        ok = ok && make_tmap<T, 3>(s, &tm_in, ec, Lc.g, TL::CW, TL::CR) && make_tmap<T, 3>(s, &tm_ac, ac, Lc.g, TL::CW, TL::CR);
+        ok = ok && make_tmap<T, ND>(s, &tm_in, ec, Lc.g, TL::CBW, TL::CR) && make_tmap<T, ND>(s, &tm_ac, ac, Lc.g, TL::CBW, TL::CR);
     } else {
-        ok = ok && make_tmap<T, 3>(s, &tm_in, in, Lt.g, TL::TXN, TL::PY);
+        ok = ok && make_tmap<T, ND>(s, &tm_in, in, Lt.g, TL::BW, TL::PY);
         tm_ac = tm_in;
     }
     if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
     const LevelGeom& g = Lt.g;
-    const int interior = std::max(g.nz - 2, 1);
-    const int tx = (g.nx - 1 + TL::OX - 1) / TL::OX, ty = (g.ny - 1 + TL::OY - 1) / TL::OY;
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const int interior = std::max(NM - 2, 1);
+    const int tx = (g.nx - 1 + TL::OX - 1) / TL::OX, ty = ND == 3 ? (g.ny - 1 + TL::OY - 1) / TL::OY : 1;
     const long long tiles = (long long)tx * ty;
-    // z chunks: one CTA per SM; pick the count that minimises waves x (planes per chunk + pipeline fill)
+    // chunks of the marching axis: pick the count that minimises waves x (planes per chunk + pipeline fill)
+    const long long slots = (long long)s->sm_count * TL::CTAS;
     int best = 1;
     double bestc = 1e300;
-    for (int nch = 1; nch <= 64 && nch <= interior; ++nch) {
+    for (int nch = 1; nch <= 256 && nch <= interior; ++nch) {
         const int mc = (interior + nch - 1) / nch;
-        const long long waves = (tiles * nch + s->sm_count - 1) / s->sm_count;
+        const long long waves = (tiles * nch + slots - 1) / slots;
         const double c = double(waves) * double(mc + 2 * NS + 6);
         if (c < bestc) { bestc = c; best = nch; }
     }
     int mc = s->march_chunk > 0 ? std::min(s->march_chunk, interior) : (interior + best - 1) / best;
     const int nch = (interior + mc - 1) / mc;
-    dim3 grid(tx, ty, nch);
-    klaunch(R, k_visit3<T, NS, INTERP>, grid, TL::NT, visit_smem_bytes<T, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
+    dim3 grid(tx, ND == 3 ? ty : nch, ND == 3 ? nch : 1);
+    klaunch(R, k_visit<T, ND, NS, INTERP>, grid, TL::NT, visit_smem_bytes<T, ND, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
             make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
 }
 
-template <class T, bool INTERP>
-void launch_visit3_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
-                      int a_assign, const T* d0, const T* v0, T* u) {
-    if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
-    else if (ns == 3) launch_visit3<T, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
-    else launch_visit3<T, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+template <class T, int ND, bool INTERP>
+void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
+                     int a_assign, const T* d0, const T* v0, T* u) {
+    if (ns == 2) launch_visit<T, ND, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+    else if (ns == 3) launch_visit<T, ND, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+    else launch_visit<T, ND, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
 }
-
 
 // launches the pending run of coarse-level operations as ONE cluster (K_coarse)
 template <class T, int ND, bool VAR>
@@ -515,7 +516,7 @@ void rec_cycle(Rec& R) {
         }
         // K_visit: the whole visit (or, on level 0, chunks of up to 4 sweeps) in one pass over HBM
         const int maxns = std::min(s->fuse_visit, 4);
-        if (ND == 3 && !VAR && maxns >= 2 && tiled(s, t) && !small(t) && eta >= 2 && (t == 0 || eta <= maxns)) {
+        if (!VAR && maxns >= 2 && tiled(s, t) && !small(t) && eta >= 2 && (t == 0 || eta <= maxns)) {
             flush();
             const int v0i = Lt.e;
             int in = v0i, i1 = -1, i2 = -1, done = 0;           // rot indices of v^k, v^{k-1}, v^{k-2}
@@ -543,10 +544,10 @@ void rec_cycle(Rec& R) {
                 const int tag = t == 0 ? TAG_VISIT0 : TAG_VISIT;
                 if (!R.plan) {
                     if (interp)
-                        launch_visit3_ns<T, true>(R, ns, t, nullptr, fuse_ec, (const T*)L[t + 1].a, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                        launch_visit_ns<T, ND, true>(R, ns, t, nullptr, fuse_ec, (const T*)L[t + 1].a, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
                                                   nullptr, 0, nullptr, nullptr, addu ? (T*)s->u : nullptr);
                     else
-                        launch_visit3_ns<T, false>(R, ns, t, rotp<T>(Lt, in), nullptr, nullptr, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                        launch_visit_ns<T, ND, false>(R, ns, t, rotp<T>(Lt, in), nullptr, nullptr, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
                                                    book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, (book && have_d0) ? (const T*)Lt.d0 : nullptr,
                                                    rotp<T>(Lt, v0i), addu ? (T*)s->u : nullptr);
                 }
@@ -681,13 +682,18 @@ cudaError_t set_attr() {
                                 res_smem_bytes<T, ND, VAR>());
 }
 
+template <class T, int ND, int NS>
+cudaError_t set_attr_visit1() {
+    cudaError_t e = cudaFuncSetAttribute(k_visit<T, ND, NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         visit_smem_bytes<T, ND, NS, false>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_visit<T, ND, NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                visit_smem_bytes<T, ND, NS, true>());
+}
 template <class T, int NS>
 cudaError_t set_attr_visit() {
-    cudaError_t e = cudaFuncSetAttribute(k_visit3<T, NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         visit_smem_bytes<T, NS, false>());
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_visit3<T, NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                visit_smem_bytes<T, NS, true>());
+    cudaError_t e = set_attr_visit1<T, 2, NS>();
+    return e != cudaSuccess ? e : set_attr_visit1<T, 3, NS>();
 }
 
 }  // namespace

@@ -28,33 +28,44 @@
 
 namespace homg {
 
-template <class T, int NS>
+template <class T, int ND, int NS>
 struct VisitTile {
     static constexpr int ES = int(sizeof(T));
     static constexpr int VEC = 16 / ES;
-    static constexpr int PX = 16, PY = 32, NT = PX * PY;      // packs per row, rows, threads
+    // 3-D: 16 packs x 32 rows per plane.  2-D: the marching axis is y, a "plane" is one row segment of
+    // 160 packs (a width that is NOT close to a power of two: 2^k+1 grids then tile with little waste).
+    static constexpr int PX = ND == 3 ? 16 : 160, PY = ND == 3 ? 32 : 1, NT = PX * PY;
+    static constexpr int CTAS = ND == 3 ? 1 : 2;              // CTAs per SM (launch bound)
     static constexpr int HX = (NS + VEC - 1) / VEC * VEC;     // x halo (nodes), pack granular
-    static constexpr int HY = NS;
+    static constexpr int HY = ND == 3 ? NS : 0;
     static constexpr int TXN = PX * VEC;                      // tile width in nodes
     static constexpr int OX = TXN - 2 * HX, OY = PY - 2 * HY; // nodes stored per plane
-    static constexpr int RS = TXN;                            // row stride (elements) = 256 B
-    static constexpr int PLANE = (PY + 2) * RS;               // one pad row below and one above
+    static constexpr int RS = TXN;                            // row stride (elements), a multiple of 128 B
+    // padded plane: 3-D one pad row below and above; 2-D 128 B before and after the row
+    static constexpr int ROFF = ND == 3 ? RS : 128 / ES;      // where the tile starts inside a padded plane
+    static constexpr int PLANE = PY * RS + 2 * ROFF;
     static constexpr int PLANE_BYTES = PLANE * ES;
-    static constexpr int BOX_BYTES = PY * RS * ES;            // one TMA box {TXN, PY, 1}
+    static constexpr int BOX_BYTES = PY * RS * ES;            // bytes of one fine plane of the tile
+    static constexpr int BW = ND == 3 ? TXN : 160;            // TMA box width (<= 256 elements); TXN / BW boxes per plane
     static constexpr int NIN = 4;                             // TMA ring depth of the v^0 planes
     static constexpr int NGR = 8;                             // g ring: plane z0-s is read by stage s (NS <= 4)
     // coarse tiles of e_c and a_c (INTERP)
     static constexpr int CWN = TXN / 2 + 1;                   // coarse columns a tile row needs
-    static constexpr int CW = (CWN + 2 * (VEC - 1)) / VEC * VEC;   // + slack: the box starts 16-B aligned
-    static constexpr int CR = PY / 2 + 2;
+    // + slack: the box starts 16-B aligned.  2-D: three boxes of 512 B
+    static constexpr int CBW = ND == 3 ? (CWN + 2 * (VEC - 1)) / VEC * VEC : 512 / ES;
+    static constexpr int NCB = ND == 3 ? 1 : 3;
+    static constexpr int CW = CBW * NCB;
+    static constexpr int CR = ND == 3 ? PY / 2 + 2 : 1;
     static constexpr int CBOX_BYTES = CR * CW * ES;
     static constexpr int CTILE_BYTES = (CBOX_BYTES + 127) / 128 * 128;
     static constexpr int NC = 4;
+    static_assert(CW >= CWN + VEC - 1, "coarse tile too narrow");
+    static_assert(PLANE_BYTES % 128 == 0 && BOX_BYTES % 128 == 0 && (BW * ES) % 128 == 0, "TMA destinations are 128-B aligned");
 };
 
-template <class T, int NS, bool INTERP>
+template <class T, int ND, int NS, bool INTERP>
 __host__ __device__ constexpr int visit_smem_bytes() {
-    using TL = VisitTile<T, NS>;
+    using TL = VisitTile<T, ND, NS>;
     return TL::NGR * TL::BOX_BYTES +
            (INTERP ? TL::NC * 2 * TL::CTILE_BYTES + NS * 2 * TL::PLANE_BYTES
                    : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + 128;
@@ -63,20 +74,23 @@ __host__ __device__ constexpr int visit_smem_bytes() {
 // tm_in : PLAIN: v^0 of this level, box {TXN, PY, 1};  INTERP: e_c of level c = t+1, box {CW, CR, 1}
 // tm_ac : INTERP: a_c, same box;  tm_g : g of this level, box {TXN, PY, 1}
 // o0 / o1 / o2 : v^NS, v^{NS-1}, v^{NS-2} (each may be null);  a, a_assign, d0, v0, u : as k_relax
-// grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior planes)
-template <class T, int NS, bool INTERP>
-__global__ void __launch_bounds__(VisitTile<T, NS>::NT, 1)
-k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
+// grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior planes);  2-D: (x tiles, y chunks)
+// ("z" / "plane" below = the marching axis: z in 3-D, y in 2-D)
+template <class T, int ND, int NS, bool INTERP>
+__global__ void __launch_bounds__(VisitTile<T, ND, NS>::NT, VisitTile<T, ND, NS>::CTAS)
+k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
          const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
          T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
          const T* __restrict__ v0, T* __restrict__ u, int mchunk) {
     pdl_start();
-    using TL = VisitTile<T, NS>;
+    using TL = VisitTile<T, ND, NS>;
     constexpr int VEC = TL::VEC, RS = TL::RS;
     const int tid = threadIdx.x, px = tid % TL::PX, py = tid / TL::PX;
-    const int x0 = blockIdx.x * TL::OX, y0 = blockIdx.y * TL::OY;
-    const int ms = 1 + blockIdx.z * mchunk;
-    const int me = min(ms + mchunk, g.nz - 1);
+    const int NM = ND == 3 ? g.nz : g.ny;
+    const long long mstride = ND == 3 ? g.pp : (long long)g.px;
+    const int x0 = blockIdx.x * TL::OX, y0 = ND == 3 ? blockIdx.y * TL::OY : 0;
+    const int ms = 1 + (ND == 3 ? blockIdx.z : blockIdx.y) * mchunk;
+    const int me = min(ms + mchunk, NM - 1);
     if (ms >= me) return;
     const int zs = ms - NS;                                        // first plane of stage 0
     const int nsteps = me - ms + 2 * NS;                           // one stage-0 plane per step
@@ -111,16 +125,29 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         const int st = q & (TL::NIN - 1), sg = q & (TL::NGR - 1), p = zs + q;
         if (!INTERP) {
             mbar_arrive_expect_tx(&fbar[st], TL::BOX_BYTES);
-            tma_load_3d(vring(st) + RS, &tm_in, &fbar[st], x0 - TL::HX, y0 - TL::HY, p);
+            if (ND == 3) tma_load_3d(vring(st) + TL::ROFF, &tm_in, &fbar[st], x0 - TL::HX, y0 - TL::HY, p);
+            else
+                for (int b = 0; b < TL::TXN / TL::BW; ++b)
+                    tma_load_2d(vring(st) + TL::ROFF + b * TL::BW, &tm_in, &fbar[st], x0 - TL::HX + b * TL::BW, p);
         }
         mbar_arrive_expect_tx(&gbar[sg], TL::BOX_BYTES);
-        tma_load_3d(gs(sg), &tm_g, &gbar[sg], x0 - TL::HX, y0 - TL::HY, p);
+        if (ND == 3) tma_load_3d(gs(sg), &tm_g, &gbar[sg], x0 - TL::HX, y0 - TL::HY, p);
+        else
+            for (int b = 0; b < TL::TXN / TL::BW; ++b)
+                tma_load_2d(gs(sg) + b * TL::BW, &tm_g, &gbar[sg], x0 - TL::HX + b * TL::BW, p);
     };
     auto issue_c = [&](int zc) {                                   // coarse plane Zc0+zc of e_c and a_c
         const int st = zc & (TL::NC - 1);
         mbar_arrive_expect_tx(&cbar[st], 2 * TL::CBOX_BYTES);
-        tma_load_3d(ce(st), &tm_in, &cbar[st], Xa, Yc, Zc0 + zc);
-        tma_load_3d(ca(st), &tm_ac, &cbar[st], Xa, Yc, Zc0 + zc);
+        if (ND == 3) {
+            tma_load_3d(ce(st), &tm_in, &cbar[st], Xa, Yc, Zc0 + zc);
+            tma_load_3d(ca(st), &tm_ac, &cbar[st], Xa, Yc, Zc0 + zc);
+        } else {
+            for (int b = 0; b < TL::NCB; ++b) {
+                tma_load_2d(ce(st) + b * TL::CBW, &tm_in, &cbar[st], Xa + b * TL::CBW, Zc0 + zc);
+                tma_load_2d(ca(st) + b * TL::CBW, &tm_ac, &cbar[st], Xa + b * TL::CBW, Zc0 + zc);
+            }
+        }
     };
     if (tid == 0) {
         if (INTERP)
@@ -130,18 +157,18 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
 
     // ---- this thread's pack: nodes x .. x+VEC-1 of row y ----
     const int x = x0 - TL::HX + px * VEC;
-    const int y = y0 - TL::HY + py;
-    const int off = (py + 1) * RS + px * VEC;                      // in a padded plane
+    const int y = y0 - TL::HY + py;                                // 2-D: 0, unused
+    const int off = TL::ROFF + py * RS + px * VEC;                 // in a padded plane
     const int goff = py * RS + px * VEC;
-    const bool row_int = y > 0 && y < g.ny - 1;
+    const bool row_int = ND == 2 || (y > 0 && y < g.ny - 1);
     bool xin[VEC];
 #pragma unroll
     for (int j = 0; j < VEC; ++j) xin[j] = row_int && (x + j > 0) && (x + j < g.nx - 1);
-    const bool own = px * VEC >= TL::HX && px * VEC < TL::HX + TL::OX && x < g.nx && py >= TL::HY &&
-                     py < TL::HY + TL::OY && y < g.ny;
+    const bool own = px * VEC >= TL::HX && px * VEC < TL::HX + TL::OX && x < g.nx &&
+                     (ND == 2 || (py >= TL::HY && py < TL::HY + TL::OY && y < g.ny));
     // INTERP: my first coarse node inside a coarse tile
-    const int yl = (y >> 1) - Yc;
-    const bool yodd = y & 1;
+    const int yl = ND == 3 ? (y >> 1) - Yc : 0;
+    const bool yodd = ND == 3 && (y & 1);
     const int coff = yl * TL::CW + (Xc - Xa) + px * (VEC / 2);
 
     // S3a in registers: the pack of v^0 at fine plane z from the coarse planes z>>1 and (z+1)>>1;
@@ -196,7 +223,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         for (int j = 0; j < VEC; ++j) { P[s].v[j] = T(0); C[s].v[j] = T(0); }
 
     // address of (x, y) in the plane the LAST stage produces at step q: z = zs + q - NS
-    long long cF = (long long)(zs - NS) * g.pp + (long long)y * g.px + x;
+    long long cF = (long long)(zs - NS) * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
 
     // STEADY: the pipeline is full and every stage's plane is interior — no range checks
     auto step = [&](auto KC, auto SD, const int q) {
@@ -224,14 +251,21 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         for (int s = 1; s <= NS; ++s) {
             // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
             const T* ctr = (s == 1 && !INTERP) ? vring(SC) : buf(s - 1, R);
-            const Pack<T> dn = *reinterpret_cast<const Pack<T>*>(ctr + off - RS);
-            const Pack<T> up = *reinterpret_cast<const Pack<T>*>(ctr + off + RS);
+            Pack<T> dn, up;
+            if (ND == 3) {
+                dn = *reinterpret_cast<const Pack<T>*>(ctr + off - RS);
+                up = *reinterpret_cast<const Pack<T>*>(ctr + off + RS);
+            }
             const Pack<T> cu = C[s - 1], pv = P[s - 1];
             const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
-            const T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
-            const T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
+            T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
+            T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
+            if (ND == 2) {                                         // a row spans several warps
+                if ((tid & 31) == 0) vl = ctr[off - 1];
+                if ((tid & 31) == 31) vr = ctr[off + VEC];
+            }
             const int z = z0 - s;
-            const bool zin = STEADY || (z > 0 && z < g.nz - 1);
+            const bool zin = STEADY || (z > 0 && z < NM - 1);
             Pack<T> out;
 #pragma unroll
             for (int j = 0; j < VEC; ++j) {
@@ -239,7 +273,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
                 const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
                 T sm = pv.v[j] + nx.v[j];
-                sm += dn.v[j] + up.v[j];
+                if (ND == 3) sm += dn.v[j] + up.v[j];
                 sm += xm + xp;
                 const T Av = (cf.twod * vc - sm) * cf.ih2;
                 const T num = cf.w * (gv.v[j] - Av);
@@ -251,9 +285,9 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             }
             if (s < NS) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
             if (s == NS - 2 && s >= 1 && o2 != nullptr && own && (STEADY || (q >= 2 * NS - 2 && q <= nsteps - 3)))
-                *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * g.pp) = out;
+                *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * mstride) = out;
             if (s == NS - 1 && s >= 1 && o1 != nullptr && own && (STEADY || (q >= 2 * NS - 1 && q <= nsteps - 2)))
-                *reinterpret_cast<Pack<T>*>(o1 + cF + g.pp) = out;
+                *reinterpret_cast<Pack<T>*>(o1 + cF + mstride) = out;
             if (s == NS && fin) {
                 if (o0) *reinterpret_cast<Pack<T>*>(o0 + cF) = out;
                 if (a) {                                           // S3e: a (+)= d0 + v^{NS-1} - v^0
@@ -283,13 +317,13 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 if (zc < ncz) issue_c(zc);
             }
         }
-        cF += g.pp;
+        cF += mstride;
     };
     using I0 = std::integral_constant<int, 0>;
     using I1 = std::integral_constant<int, 1>;
     for (int q = 0; q < nsteps; q += 2) {
         // steps q and q+1 are steady when all their stores are due and planes z0-NS .. z0-1 are interior
-        const bool steady = q >= 2 * NS && q + 1 <= nsteps - 3 && zs + q - NS >= 1 && zs + q <= g.nz - 2;
+        const bool steady = q >= 2 * NS && q + 1 <= nsteps - 3 && zs + q - NS >= 1 && zs + q <= NM - 2;
         if (steady) {
             step(I0{}, std::true_type{}, q);
             step(I1{}, std::true_type{}, q + 1);
