@@ -9,7 +9,7 @@
 // What is here (PAPER.md line numbers; DESIGN.md lists every reading R1..):
 //   apply_A / residual       A = -div(k grad) on a 5-/7-point stencil, Dirichlet u=0
 //                            (Eq.1, L89-93 Eq.4; sign: DESIGN.md R1)
-//   jacobi                   damped Jacobi v <- v + w D^-1 (g - A v)   (L53-67 Eq.2-3)
+//   jacobi                   damped Jacobi, Eq. 3: v <- v + w_p ((sum_nb v - 2d v) + h^2 g)   (L53-67 Eq.2-3)
 //   restrict_fw              weighted-average restriction P, nested (L47, L67, L73)
 //   prolong                  linear (bi-/tri-linear) interpolation S     (L47, L51)
 //   homg  alg=0 "L"          the literal single-array HOMG iteration: every whole-grid
@@ -122,9 +122,21 @@ inline T diag_node(int nd, const T* kc, int64_t c, const int64_t st[3], T ih2) {
     return acc * ih2;
 }
 
-// damped Jacobi at one node:  v + w (g - A v) / D
+// damped Jacobi at one node.
+//   constant coefficient: Eq. 3 (L65) as printed, in the sign convention of DESIGN.md R1 (A = -lap,
+//   g = the paper's -P_m f):   v + w_p ((sum_nb v - 2d v) + h_l^2 g),   w_p = w / 2d,  h2 = h_l^2.
+//   The three multiply-adds are single fused operations (std::fma), in Eq. 3's order: neighbour sum
+//   minus 2d v, plus h^2 g, times w_p, added to v (R14; the GPU uses FMA in the same places).
+//   nodal coefficient k: no equation in the paper; v + w (g - A v) / D with the flux-form A, D (R11).
 template <class T>
-inline T jacobi_node(int nd, const T* v, const T* kc, int64_t c, const int64_t st[3], T ih2, T w, T g) {
+inline T jacobi_node(int nd, const T* v, const T* kc, int64_t c, const int64_t st[3], T ih2, T w, T g, T h2, T wp) {
+    if (!kc) {
+        T s = 0;
+        for (int a = 3 - nd; a < 3; ++a) s += v[c - st[a]] + v[c + st[a]];
+        T t = std::fma(-T(2 * nd), v[c], s);
+        t = std::fma(h2, g, t);
+        return std::fma(wp, t, v[c]);
+    }
     T Av = opA_node(nd, v, kc, c, st, ih2);
     T D = diag_node(nd, kc, c, st, ih2);
     return v[c] + w * (g - Av) / D;
@@ -160,11 +172,12 @@ template <class T>
 void jacobi(const Grid& G, double h, const T* kc, double omega, const T* v, const T* g, T* out) {
     T ih2 = T(1.0 / (h * h));
     T w = T(omega);
+    T h2 = T(h * h), wp = T(omega / double(2 * G.nd));
     FOR_NODES(G, p) {
         int64_t p[3] = {p0, p1, p2};
         int64_t c = G.idx(p);
         if (G.on_boundary(p)) { out[c] = 0; continue; }
-        out[c] = jacobi_node(G.nd, v, kc, c, G.st, ih2, w, g[c]);
+        out[c] = jacobi_node(G.nd, v, kc, c, G.st, ih2, w, g[c], h2, wp);
         ++g_relax_updates;
     }
 }
@@ -313,6 +326,7 @@ void iteration_L(const Hier<T>& H, int m, double omega, const std::vector<T>& gm
     int64_t stl[3] = {F.st[0] * l, F.st[1] * l, F.st[2] * l};
     T ih2 = T(1.0 / (H.h[m] * H.h[m]));
     T w = T(omega);
+    T h2 = T(H.h[m] * H.h[m]), wp = T(omega / double(2 * nd));
     const T* kc = H.kptr(0);
     // variation of every node in the previous iteration
     for (int64_t i = 0; i < F.size(); ++i) var[i] = cur[i] - prev[i];
@@ -324,7 +338,7 @@ void iteration_L(const Hier<T>& H, int m, double omega, const std::vector<T>& gm
         if (lattice) {
             if (F.on_boundary(p)) { nxt[c] = 0; continue; }
             int64_t P[3] = {p[0] / l, p[1] / l, p[2] / l};
-            nxt[c] = jacobi_node(nd, cur.data(), kc, c, stl, ih2, w, gm[Gm.idx(P)]);
+            nxt[c] = jacobi_node(nd, cur.data(), kc, c, stl, ih2, w, gm[Gm.idx(P)], h2, wp);
             ++g_relax_updates;
         } else {
             nxt[c] = cur[c] + interp_node(nd, p, l, var.data(), stl);

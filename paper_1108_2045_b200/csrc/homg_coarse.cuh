@@ -161,9 +161,19 @@ __device__ __forceinline__ void coarse_node(const CoarseOp<T>& o, int x, int y, 
             return;
         }
         const T vc = ldcg(o.p[0] + c);
-        T Av, D;
-        cnode_A<T, ND, VAR, CG>(o.p[0], o.p[2], c, g, o.cf, vc, Av, D);
-        T vn = vc + o.cf.w * (ldcg(o.p[1] + c) - Av) / D;
+        T vn;
+        if (!VAR) {
+            const T* v = o.p[0];
+            T s = T(0);
+            if (ND == 3) s += ldcg(v + c - g.pp) + ldcg(v + c + g.pp);
+            s += ldcg(v + c - g.px) + ldcg(v + c + g.px);
+            s += ldcg(v + c - 1) + ldcg(v + c + 1);
+            vn = jacobi_eq3(vc, s, ldcg(o.p[1] + c), o.cf);
+        } else {
+            T Av, D;
+            cnode_A<T, ND, VAR, CG>(o.p[0], o.p[2], c, g, o.cf, vc, Av, D);
+            vn = vc + o.cf.w * (ldcg(o.p[1] + c) - Av) / D;
+        }
         vout[c] = vn;
         if (a) {
             T Dq = ((o.p[3] ? ldcg(o.p[3] + c) : T(0)) + vc) - ldcg(o.p[4] + c);

@@ -118,6 +118,8 @@ Coef<T> make_coef(const homg_solver* s, int m) {
     c.D = d;
     volatile T rd = T(1) / d;               // IEEE division: RN(1/D)
     c.rD = rd;
+    c.h2 = T(h * h);
+    c.wp = T(s->omega / double(2 * s->ndim));
     return c;
 }
 

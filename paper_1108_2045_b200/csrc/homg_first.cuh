@@ -254,13 +254,12 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
                 const T vc = cur.v[j];
                 const T xm = j == 0 ? vl : cur.v[j - 1 < 0 ? 0 : j - 1];
                 const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-                T Av, D;
+                T Av = T(0), D = T(1), eq3 = T(0);
                 if (!VAR) {
                     T s = prv.v[j] + nxt.v[j];
                     if (ND == 3) s += dn.v[j] + up.v[j];
                     s += xm + xp;
-                    Av = (cf.twod * vc - s) * cf.ih2;
-                    D = cf.D;
+                    eq3 = jacobi_eq3(vc, s, gv.v[j], cf);
                 } else {
                     const T kc = kcur.v[j];
                     const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
@@ -277,8 +276,7 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
                     Av = acc * cf.ih2;
                     D = ds * cf.ih2;
                 }
-                const T num = cf.w * (gv.v[j] - Av);
-                out.v[j] = xin[j] ? vc + (VAR ? num / D : div_const(num, cf.D, cf.rD)) : T(0);
+                out.v[j] = xin[j] ? (VAR ? vc + cf.w * (gv.v[j] - Av) / D : eq3) : T(0);
             }
             if (owned) {
                 if (vout) *reinterpret_cast<Pack<T>*>(vout + c) = out;

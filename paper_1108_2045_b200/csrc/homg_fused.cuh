@@ -27,8 +27,6 @@ template <class T>
 struct alignas(2 * sizeof(T)) HalfPack {
     T v[2];
 };
-__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
-__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 // x / D for a per-level constant D with rD = RN(1/D) precomputed on the host: q = RN(x rD),
 // r = x - q D (exact in one FMA), result RN(q + r rD).  By Markstein's theorem this is the correctly
@@ -181,13 +179,12 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
             const T vc = cur.v[j];
             const T xm = j == 0 ? vl : cur.v[j - 1 < 0 ? 0 : j - 1];
             const T xp = j == VEC - 1 ? vr : cur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-            T Av, D;
+            T Av = T(0), D = T(1), eq3 = T(0);
             if (!VAR) {
                 T s = prv.v[j] + nxt.v[j];
                 if (ND == 3) s += dn.v[j] + up.v[j];
                 s += xm + xp;
-                Av = (cf.twod * vc - s) * cf.ih2;
-                D = cf.D;
+                eq3 = jacobi_eq3(vc, s, gv.v[j], cf);
             } else {
                 const T kc = kcur.v[j];
                 const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
@@ -204,8 +201,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
                 Av = acc * cf.ih2;
                 D = ds * cf.ih2;
             }
-            const T num = cf.w * (gv.v[j] - Av);
-            out.v[j] = xin[j] ? vc + (VAR ? num / D : div_const(num, cf.D, cf.rD)) : T(0);
+            out.v[j] = xin[j] ? (VAR ? vc + cf.w * (gv.v[j] - Av) / D : eq3) : T(0);
         }
         if (row_ok) {
             if (vout) *reinterpret_cast<Pack<T>*>(vout + c) = out;

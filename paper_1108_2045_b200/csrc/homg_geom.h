@@ -17,6 +17,8 @@ struct Coef {            // per-level operator constants
     T twod;              // 2d
     T D;                 // 2d * (1/h_m^2), rounded as the kernels round it (constant coefficient)
     T rD;                // RN(1/D)
+    T h2;                // h_m^2                     (Eq. 3 form of the constant-coefficient sweep)
+    T wp;                // omega / 2d
 };
 
 }  // namespace homg

@@ -72,10 +72,31 @@ __device__ __forceinline__ void node_A(const T* __restrict__ v, const T* __restr
     }
 }
 
-// damped Jacobi at one interior node: v + w (g - A v)/D
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+// constant-coefficient damped Jacobi, Eq. 3 in the sign convention of DESIGN.md R1:
+//   v + w_p ((sum_nb v - 2d v) + h_l^2 g),  w_p = w / 2d;  s = the neighbour sum (slowest axis first).
+// The three multiply-adds are single fused operations, in the same places as the oracle's std::fma
+// calls (R14), so every kernel that sweeps agrees with it bit for bit.
+template <class T>
+__device__ __forceinline__ T jacobi_eq3(T vc, T s, T gval, const Coef<T>& cf) {
+    T t = fma_rn(-cf.twod, vc, s);
+    t = fma_rn(cf.h2, gval, t);
+    return fma_rn(cf.wp, t, vc);
+}
+
+// damped Jacobi at one interior node
 template <class T, int ND, bool VAR>
 __device__ __forceinline__ T node_jacobi(const T* __restrict__ v, const T* __restrict__ k, T gval,
                                          long long c, const LevelGeom& g, const Coef<T>& cf) {
+    if (!VAR) {
+        T s = T(0);
+        if (ND == 3) s += v[c - g.pp] + v[c + g.pp];
+        s += v[c - g.px] + v[c + g.px];
+        s += v[c - 1] + v[c + 1];
+        return jacobi_eq3(v[c], s, gval, cf);
+    }
     T Av, D;
     node_A<T, ND, VAR>(v, k, c, g, cf, Av, D);
     return v[c] + cf.w * (gval - Av) / D;

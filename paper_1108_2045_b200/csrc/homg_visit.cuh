@@ -275,9 +275,7 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
                 T sm = pv.v[j] + nx.v[j];
                 if (ND == 3) sm += dn.v[j] + up.v[j];
                 sm += xm + xp;
-                const T Av = (cf.twod * vc - sm) * cf.ih2;
-                const T num = cf.w * (gv.v[j] - Av);
-                out.v[j] = xin[j] ? vc + div_const(num, cf.D, cf.rD) : T(0);
+                out.v[j] = xin[j] ? jacobi_eq3(vc, sm, gv.v[j], cf) : T(0);
             }
             if (!zin) {                                            // Dirichlet planes z = 0, nz-1 (and beyond)
 #pragma unroll
