@@ -91,7 +91,13 @@ typedef struct {
     int march_chunk;  /* planes per CTA along the marching axis of the tiled kernels; <= 0:
                          chosen from the SM count                  */
     void* cuda_stream; /* cudaStream_t; NULL = legacy default stream                     */
+    int cycle;        /* HOMG_CYCLE_MFMG (0, default): the paper's high-occupancy cycle;
+                         HOMG_CYCLE_V (1): the classic V(v_eta1, v_eta2) cycle of PAPER.md L47 on the
+                         same hierarchy, operators and kernels (exact solve on the coarsest level,
+                         which must then have exactly one interior node); schedule/max_iters unused */
+    int v_eta1, v_eta2; /* pre-/post-smoothing sweeps of HOMG_CYCLE_V; < 0: 2 and 1          */
 } homg_options;
+enum { HOMG_CYCLE_MFMG = 0, HOMG_CYCLE_V = 1 };
 
 /* Fills *opt with the defaults (all "use default" markers). */
 HOMG_API void homg_default_options(homg_options* opt);

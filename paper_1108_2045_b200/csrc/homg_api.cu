@@ -67,6 +67,7 @@ void homg_default_options(homg_options* o) {
     std::memset(o, 0, sizeof(*o));
     o->omega = 0; o->h = 0; o->max_iters = 0; o->schedule = HOMG_SCHED_C;
     o->coarse_threshold_nodes = 0; o->use_graph = -1; o->history_cap = 0; o->cuda_stream = nullptr;
+    o->cycle = HOMG_CYCLE_MFMG; o->v_eta1 = -1; o->v_eta2 = -1;
 }
 
 size_t homg_workspace_bytes(int ndim, const int64_t* dims, int levels, homg_stencil st, homg_dtype dt) {
@@ -109,12 +110,23 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (const char* ev = std::getenv("HOMG_PDL")) s->pdl = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
+    s->vcycle = o.cycle == HOMG_CYCLE_V;
+    s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;
+    s->v_eta2 = o.v_eta2 >= 0 ? o.v_eta2 : 1;
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);
     s->hist_cap = hist_cap;
     if (build_schedule(o.schedule, levels, s->max_iters, o.sched_levels, o.sched_iters, o.sched_len, s->sched_lv,
                        s->sched_it, &why) < 0) {
         delete s;
         return set_err(nullptr, HOMG_EINVAL, why);
+    }
+    if (s->vcycle) {
+        bool one = true;
+        for (int a = 0; a < ndim; ++a) one = one && ((dims[a] - 1) >> (levels - 1)) == 2;
+        if (!one || levels < 2) {
+            delete s;
+            return set_err(nullptr, HOMG_EINVAL, "HOMG_CYCLE_V needs >= 2 levels and a coarsest level of 3 nodes per axis");
+        }
     }
     // ---- carve the workspace ----
     s->ws_base = static_cast<char*>(ws); s->ws_bytes = ws_bytes;

@@ -31,6 +31,8 @@ struct Rec {                 // bookkeeping while recording
     int last_tag = TAG_OTHER;
     double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class (per sweep)
     double comp_tag[TAG_COUNT] = {};          // compulsory bytes per kernel class (what the launch must move)
+    const void* g_override = nullptr;         // V-cycle, level 0: the sweeps' right-hand side is f, not g_0
+    const void* u_override = nullptr;         // V-cycle: the residual is taken of this iterate instead of u
     bool plan = false;                        // planning pass: build the coarse program, launch nothing
     std::vector<unsigned char> prog;          // CoarseOp records of the whole cycle, in order
     int prog_nops = 0, run_begin = 0, run_len = 0;
@@ -180,7 +182,7 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
         using TL = Tile<T, ND>;
         CUtensorMap tmv, tmg, tmk;
         bool ok = make_tmap<T, ND>(s, &tmv, vin, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1) &&
-                  make_tmap<T, ND>(s, &tmg, Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
+                  make_tmap<T, ND>(s, &tmg, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
         if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, Lt.k, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1);
         else tmk = tmv;
         if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
@@ -191,7 +193,7 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
         klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
                                                                                       d0, v0, u, mc);
     } else {
-        klaunch(R, k_relax<T, ND, VAR>, grd(Lt.g), blk(), 0, Lt.g, cf, vin, (const T*)Lt.gsrc, (const T*)Lt.k, vout, a,
+        klaunch(R, k_relax<T, ND, VAR>, grd(Lt.g), blk(), 0, Lt.g, cf, vin, (const T*)(R.g_override ? R.g_override : Lt.gsrc), (const T*)Lt.k, vout, a,
                                                             a_assign, d0, v0, u);
     }
 }
@@ -238,7 +240,7 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
     Level& Lt = s->L[t];
     using TL = VisitTile<T, ND, NS>;
     CUtensorMap tm_in, tm_ac, tm_g;
-    bool ok = make_tmap<T, ND>(s, &tm_g, Lt.gsrc, Lt.g, TL::BW, TL::PY);
+    bool ok = make_tmap<T, ND>(s, &tm_g, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::BW, TL::PY);
     if (INTERP) {
         Level& Lc = s->L[t + 1];
         ok = ok && make_tmap<T, ND>(s, &tm_in, ec, Lc.g, TL::CBW, TL::CR) && make_tmap<T, ND>(s, &tm_ac, ac, Lc.g, TL::CBW, TL::CR);
@@ -318,7 +320,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
     if (tiled(s, 0)) {
         using TL = ResTile<T, ND>;
         CUtensorMap tmu, tmf, tmk;
-        bool ok = make_tmap<T, ND>(s, &tmu, s->u, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1) &&
+        bool ok = make_tmap<T, ND>(s, &tmu, R.u_override ? R.u_override : s->u, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1) &&
                   make_tmap<T, ND>(s, &tmf, s->f, L0.g, TL::SEG, ND == 3 ? TL::TY + 1 : 1);
         if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, L0.k, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1);
         else tmk = tmu;
@@ -345,7 +347,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         if (fused_restrict) R.acct(1, 1.0);
     } else {
         dim3 g = grd(L0.g);
-        if (!R.plan) klaunch(R, k_residual<T, ND, VAR>, g, blk(), 0, L0.g, make_coef<T>(s, 0), (const T*)s->u, (const T*)s->f,
+        if (!R.plan) klaunch(R, k_residual<T, ND, VAR>, g, blk(), 0, L0.g, make_coef<T>(s, 0), (const T*)(R.u_override ? R.u_override : s->u), (const T*)s->f,
                                                        (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
         R.check(TAG_RESIDUAL0);
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
@@ -624,6 +626,110 @@ void rec_cycle(Rec& R) {
     flush();
 }
 
+// ---------------------------------------------------------------------------------------------
+// Classic V(eta1, eta2) cycle on the same hierarchy and kernels:
+// (a) eta1 sweeps, (b) r = g - A v restricted by full weighting, (c) exact solve on the coarsest
+// level (one interior node), (d) v += S^ e, (e) eta2 sweeps.  Level 0 works on u itself with g = f.
+// ---------------------------------------------------------------------------------------------
+// n sweeps on level m starting from `cur`; the last one writes into `final_dst` when given and
+// possible.  Returns the array that holds the result.
+template <class T, int ND, bool VAR>
+T* v_sweeps(Rec& R, int m, T* cur, int n, T* final_dst) {
+    homg_solver* s = R.s;
+    Level& Lm = s->L[m];
+    auto pick = [&](const T* not1, const T* not2) -> T* {
+        for (int b = 0; b < Lm.nrot; ++b) {
+            T* c = rotp<T>(Lm, b);
+            if (c != not1 && c != not2) return c;
+        }
+        return nullptr;
+    };
+    const int maxns = std::min(s->fuse_visit, 4);
+    int done = 0;
+    while (done < n) {
+        const int rem = n - done;
+        const bool fuse = !VAR && maxns >= 2 && tiled(s, m) && rem >= 2;
+        const int ns = fuse ? std::min(rem, maxns) : 1;
+        const bool lastc = done + ns == n;
+        T* out = (lastc && final_dst && final_dst != cur) ? final_dst : pick(cur, final_dst);
+        if (fuse) {
+            launch_visit_ns<T, ND, false>(R, ns, m, cur, nullptr, nullptr, out, nullptr, nullptr, nullptr, 0, nullptr, nullptr, nullptr);
+            R.check(m == 0 ? TAG_VISIT0 : TAG_VISIT);
+            R.acct2(m, 3.0 * ns, 3.0, m == 0 ? TAG_VISIT0 : TAG_VISIT);
+        } else {
+            launch_relax<T, ND, VAR>(R, m, cur, out, nullptr, 0, nullptr, nullptr, nullptr);
+            R.check(m == 0 ? TAG_RELAX0 : TAG_RELAX);
+            R.acct(m, 3.0 + (VAR ? 1.0 : 0.0), m == 0 ? TAG_RELAX0 : TAG_RELAX);
+        }
+        cur = out;
+        done += ns;
+    }
+    return cur;
+}
+
+template <class T, int ND, bool VAR>
+void rec_vcycle(Rec& R) {
+    homg_solver* s = R.s;
+    const int M = s->levels - 1;
+    std::vector<Level>& L = s->L;
+    // norm of the current u -> history (the classic cycle has no residual of the iterate it starts from)
+    rec_norm<T, ND, VAR>(R, false, true, false);
+    std::vector<T*> cur(s->levels, nullptr);
+    cur[0] = (T*)s->u;
+    for (int m = 0; m < M; ++m) {
+        Level& Lm = L[m];
+        if (m >= 1) {                                            // e_m = 0
+            cur[m] = rotp<T>(Lm, 0);
+            cudaMemsetAsync(cur[m], 0, Lm.n_alloc * sizeof(T), R.st);
+            R.check(TAG_OTHER);
+        }
+        R.g_override = m == 0 ? s->f : nullptr;
+        cur[m] = v_sweeps<T, ND, VAR>(R, m, cur[m], s->v_eta1, nullptr);                       // (a)
+        R.g_override = nullptr;
+        if (m == 0) {                                            // (b) K_res: r -> g_0 scratch, g_1 = P r
+            R.u_override = cur[0];
+            const bool have_g1 = rec_norm<T, ND, VAR>(R, true, false, true);
+            R.u_override = nullptr;
+            if (!have_g1) {
+                klaunch(R, k_restrict<T, ND>, grd(L[1].g), blk(), 0, L[1].g, L[0].g, (const T*)L[0].gsrc, (T*)L[1].gsrc);
+                R.check(TAG_RESTRICT);
+                R.acct(0, 1.0, TAG_RESTRICT); R.acct(1, 1.0, TAG_RESTRICT);
+            }
+        } else {
+            klaunch(R, k_residual<T, ND, VAR>, grd(Lm.g), blk(), 0, Lm.g, make_coef<T>(s, m), (const T*)cur[m],
+                    (const T*)Lm.gsrc, (const T*)Lm.k, (T*)Lm.tmp, s->partial);
+            R.check(TAG_OTHER);
+            R.acct(m, 3.0 + (VAR ? 1.0 : 0.0), TAG_OTHER);
+            klaunch(R, k_restrict<T, ND>, grd(L[m + 1].g), blk(), 0, L[m + 1].g, Lm.g, (const T*)Lm.tmp, (T*)L[m + 1].gsrc);
+            R.check(TAG_RESTRICT);
+            R.acct(m, 1.0, TAG_RESTRICT); R.acct(m + 1, 1.0, TAG_RESTRICT);
+        }
+    }
+    // (c) coarsest level: exact solve (one interior node)
+    cur[M] = rotp<T>(L[M], 0);
+    if (M >= 1) {
+        cudaMemsetAsync(cur[M], 0, L[M].n_alloc * sizeof(T), R.st);
+        R.check(TAG_OTHER);
+        klaunch(R, k_coarsest_solve<T, ND, VAR>, dim3(1), dim3(32), 0, L[M].g, make_coef<T>(s, M), (const T*)L[M].gsrc,
+                (const T*)L[M].k, cur[M]);
+        R.check(TAG_COARSE);
+    }
+    for (int m = M - 1; m >= 0; --m) {
+        Level& Lm = L[m];
+        klaunch(R, k_prolong_add_v<T, ND>, grdv<T>(Lm.g), blk(), 0, Lm.g, L[m + 1].g, (const T*)cur[m + 1], cur[m]);   // (d)
+        R.check(m == 0 ? TAG_DELIVER0 : TAG_DELIVER);
+        R.acct(m, 2.0, m == 0 ? TAG_DELIVER0 : TAG_DELIVER); R.acct(m + 1, 1.0, m == 0 ? TAG_DELIVER0 : TAG_DELIVER);
+        R.g_override = m == 0 ? s->f : nullptr;
+        cur[m] = v_sweeps<T, ND, VAR>(R, m, cur[m], s->v_eta2, m == 0 ? (T*)s->u : nullptr);     // (e)
+        R.g_override = nullptr;
+    }
+    if (cur[0] != (T*)s->u) {                                    // eta2 = 0, or a single sweep that started from u
+        cudaMemcpyAsync(s->u, cur[0], L[0].n_alloc * sizeof(T), cudaMemcpyDeviceToDevice, R.st);
+        R.check(TAG_OTHER);
+        R.acct(0, 2.0, TAG_OTHER);
+    }
+}
+
 template <class T, int ND, bool VAR>
 void rec_sample(Rec& R) {
     homg_solver* s = R.s;
@@ -727,7 +833,7 @@ cudaError_t exec_init(homg_solver* s) {
 }
 
 cudaError_t exec_prepare(homg_solver* s) {
-    if (s->prog_ready) return cudaSuccess;
+    if (s->prog_ready || s->vcycle) return cudaSuccess;       // the V-cycle has no coarse program
     Rec P{s, s->stream};
     P.plan = true;
     HOMG_DISPATCH(s, rec_cycle, P);
@@ -744,7 +850,8 @@ cudaError_t exec_prepare(homg_solver* s) {
 
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     Rec R{s, st};
-    HOMG_DISPATCH(s, rec_cycle, R);
+    if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
+    else HOMG_DISPATCH(s, rec_cycle, R);
     s->launches_per_cycle = R.launches;
     s->bytes_cycle_all = R.bytes_all;
     s->bytes_cycle_l0 = R.bytes_l0;
@@ -761,7 +868,8 @@ cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_t
     cudaEventRecord(e0, st);
     Rec R{s, st};
     R.ev = &ev; R.ev_tag = &tag;
-    HOMG_DISPATCH(s, rec_cycle, R);
+    if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
+    else HOMG_DISPATCH(s, rec_cycle, R);
     cudaError_t e = cudaStreamSynchronize(st);
     if (R.err == cudaSuccess) R.err = e;
     cudaEvent_t prev = e0;

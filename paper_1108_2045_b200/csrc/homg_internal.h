@@ -70,6 +70,8 @@ struct homg_solver {
     int march_chunk = 0;             // 0: automatic
     bool pdl = true;                 // programmatic dependent launch on every kernel (HOMG_PDL=0 disables)
     bool fuse_first = true;          // fused interpolate+correct+relax first sweep (HOMG_FUSE_FIRST=0 disables)
+    bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
+    int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create

@@ -114,4 +114,44 @@ k_d0_down_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, const T* __rest
     *reinterpret_cast<Pack<T>*>(out + lidx(gf, x, y, z)) = val;
 }
 
+// Classic V-cycle, step (d): v += S^ e_c on every node (coincident nodes add e_c itself,
+// weight 1).  One pack per thread, fine array updated in place.
+template <class T, int ND>
+__global__ void __launch_bounds__(256)
+k_prolong_add_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, T* __restrict__ v) {
+    pdl_start();
+    HOMG_PACK_XYZ(gf);
+    const long long c = lidx(gf, x, y, z);
+    const Pack<T> inc = pack_interp<T, ND>(gc, ec, nullptr, x, y, z);
+    Pack<T> vv = *reinterpret_cast<const Pack<T>*>(v + c);
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) vv.v[j] = x + j < gf.nx ? vv.v[j] + inc.v[j] : T(0);
+    *reinterpret_cast<Pack<T>*>(v + c) = vv;
+}
+
+// Classic V-cycle, step (c) on a coarsest level with ONE interior node (3^d grid): the exact solve
+// e = g / D, evaluated in double as the oracle's 1x1 LU does (D = the operator's diagonal in T).
+template <class T, int ND, bool VAR>
+__global__ void k_coarsest_solve(LevelGeom g, Coef<T> cf, const T* __restrict__ gsrc, const T* __restrict__ k,
+                                 T* __restrict__ e) {
+    pdl_start();
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const long long c = lidx(g, 1, 1, ND == 3 ? 1 : 0);
+    T D;
+    if (!VAR) {
+        D = cf.twod * cf.ih2;
+    } else {
+        const T kc = k[c];
+        T acc = T(0);
+        const long long off[3] = {g.pp, (long long)g.px, 1};
+#pragma unroll
+        for (int a = 3 - ND; a < 3; ++a) {
+            acc += kface(kc, k[c - off[a]]) * (T(1) - T(0));
+            acc += kface(kc, k[c + off[a]]) * (T(1) - T(0));
+        }
+        D = acc * cf.ih2;
+    }
+    e[c] = T(double(gsrc[c]) / double(D));
+}
+
 }  // namespace homg

@@ -30,7 +30,7 @@ class HomgOptions(C.Structure):
         ("sched_levels", C.POINTER(C.c_int)), ("sched_iters", C.POINTER(C.c_int)), ("sched_len", C.c_int),
         ("coarse_threshold_nodes", C.c_int), ("use_graph", C.c_int), ("history_cap", C.c_int),
         ("tiled_min_nodes", C.c_int), ("march_chunk", C.c_int),
-        ("cuda_stream", C.c_void_p),
+        ("cuda_stream", C.c_void_p), ("cycle", C.c_int), ("v_eta1", C.c_int), ("v_eta2", C.c_int),
     ]
 
 
@@ -98,7 +98,7 @@ class Solver:
 
     def __init__(self, dims, levels, stencil, dtype, omega=0.0, h=0.0, max_iters=0, schedule=HOMG_SCHED_C,
                  sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, tiled_min_nodes=0,
-                 march_chunk=0, device="cuda:0", stream=None):
+                 march_chunk=0, device="cuda:0", stream=None, vcycle=None):
         import torch
         self._torch = torch
         self.dims = tuple(int(x) for x in dims)
@@ -114,6 +114,8 @@ class Solver:
         o.omega, o.h, o.max_iters, o.schedule = float(omega), float(h), int(max_iters), int(schedule)
         o.coarse_threshold_nodes, o.use_graph, o.history_cap = int(coarse_threshold_nodes), int(use_graph), int(history_cap)
         o.tiled_min_nodes, o.march_chunk = int(tiled_min_nodes), int(march_chunk)
+        if vcycle is not None:                      # classic V(eta1, eta2) instead of the MFMG cycle
+            o.cycle, o.v_eta1, o.v_eta2 = 1, int(vcycle[0]), int(vcycle[1])
         self._keep = None
         if sched is not None:
             lv, it = sched

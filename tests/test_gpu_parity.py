@@ -218,3 +218,46 @@ def test_tiled_matches_generic_bitwise(orc):
     b, nb, _ = run_gpu(cfg, inp, 3, tiled_min_nodes=-1)
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+# ---- classic V(eta1, eta2) cycle on the GPU vs the oracle's Algorithm V ----
+def check_vcycle(cfg, ncycles, orc, eta=(2, 1), **kw):
+    inp = I.make_inputs(cfg)
+    us, norms, _ = run_gpu(cfg, inp, ncycles, vcycle=eta, **kw)
+    _, hist, onorms = orc.vcycle(inp["f"], inp["u0"], cfg.levels, cfg.omega, eta[0], eta[1], ncycles, k=inp["k"],
+                                 keep_history=True)
+    tol = TOL[cfg.dtype]
+    for c in range(ncycles):
+        ref = hist[c].astype(np.float64)
+        err = np.max(np.abs(us[c].astype(np.float64) - ref)) / np.max(np.abs(ref))
+        assert err <= tol, f"{cfg.name} V{eta}: cycle {c}: max-norm relative difference {err:.3e} > {tol}"
+    floor = 1e-11 if cfg.dtype == "f64" else 3e-5
+    for c in range(1, ncycles + 1):
+        if onorms[c] / onorms[0] < floor:
+            break
+        fg, fo = norms[c] / norms[c - 1], onorms[c] / onorms[c - 1]
+        assert abs(fg - fo) <= 5e-3 * abs(fo), (cfg.name, c, fg, fo)
+    return norms
+
+
+@pytest.mark.parametrize("name,n,eta", [("cfg1", 129, (2, 1)), ("cfg2", 33, (2, 1)), ("cfg2", 65, (1, 1)), ("cfg3", 257, (2, 2)),
+                                        ("cfg4", 65, (2, 1)), ("cfg5", 33, (2, 1)), ("cfg4", 33, (0, 1)), ("cfg2", 17, (3, 0)),
+                                        ("cfg4", 129, (4, 4))])
+def test_vcycle_mode(orc, name, n, eta):
+    cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+    check_vcycle(cfg, 4, orc, eta=eta)
+
+
+def test_vcycle_tiled_every_level_and_contraction(orc):
+    """tiled kernels (K_visit, K_res) on every level; the V(2,1) factor is h-independent and ~ mu^3 (pin P11)."""
+    cfg = I.scaled(I.CONFIGS["cfg2"], 65)
+    norms = check_vcycle(cfg, 6, orc, eta=(2, 1), tiled_min_nodes=1)
+    fac = norms[5] / norms[4]
+    assert fac < 0.45, fac
+
+
+def test_vcycle_needs_one_node_coarsest_level():
+    _torch()
+    from paper_1108_2045_b200 import homg
+    with pytest.raises(homg.HomgError):
+        homg.Solver((65, 65, 65), 4, "poisson7", "f64", vcycle=(2, 1))
