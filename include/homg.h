@@ -95,7 +95,8 @@ typedef struct {
                          HOMG_CYCLE_V (1): the classic V(v_eta1, v_eta2) cycle of PAPER.md L47 on the
                          same hierarchy, operators and kernels (exact solve on the coarsest level,
                          which must then have exactly one interior node); schedule/max_iters unused */
-    int v_eta1, v_eta2; /* pre-/post-smoothing sweeps of HOMG_CYCLE_V; < 0: 2 and 1          */
+    int v_eta1;       /* pre-smoothing sweeps of HOMG_CYCLE_V; < 0: 2                    */
+    int v_eta2;       /* post-smoothing sweeps of HOMG_CYCLE_V; < 0: 1                   */
 } homg_options;
 enum { HOMG_CYCLE_MFMG = 0, HOMG_CYCLE_V = 1 };
 
