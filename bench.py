@@ -260,15 +260,13 @@ def run_reference(args):
 def run_homg(args):
     import torch
     import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
+    from paper_1108_2045_b200 import replicas
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
     dev = f"cuda:{local}"
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+    rank, world = replicas.init("nccl", torch.device(dev))
     cfg = I.CONFIGS[args.workload]
     if args.n:
         cfg = I.scaled(cfg, args.n)
@@ -286,9 +284,8 @@ def run_homg(args):
 
     def sync_all():
         torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
+        replicas.barrier()
+        torch.cuda.synchronize()
 
     for _ in range(max(3, args.warmup)):
         flush.zero_()
@@ -353,13 +350,10 @@ def run_homg(args):
     bytes_cycle = s.bytes_per_cycle()
     clocks = sampler.stop()
 
-    tt = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s = float(tt[0]), float(tt[1])
+    total_ms, e2e_s = replicas.max_over_ranks([total_ms, e2e_s], device=dev)
     es = 8 if cfg.dtype == "f64" else 4
     nbytes = int(np.prod(cfg.dims)) * es
-    line = {"metric": METRIC, "value": cfg.n_interior * args.steps * world / (total_ms * 1e-3), "unit": UNIT,
+    line = {"metric": METRIC, "value": replicas.job_value(cfg.n_interior, args.steps, world, total_ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": dict(workload_config(cfg), l2="flushed between steps (512 MiB write)",
