@@ -174,7 +174,10 @@ class Solver:
             self._ck(lib().homg_residual_history(self.handle, buf, n.value, C.byref(n)))
         return list(buf[:n.value])
 
-    def get_solution(self, out):
+    def get_solution(self, out=None):
+        if out is None:
+            import numpy as np
+            out = np.empty(self.dims, dtype=np.float64 if self.dtype == "f64" else np.float32)
         self._call_arr(lib().homg_get_solution, out)
         return out
 
