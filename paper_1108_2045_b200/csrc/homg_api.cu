@@ -145,7 +145,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
         L.gsrc = take(ab);
         for (int b = 0; b < L.nrot; ++b) L.rot[b] = take(ab);
         if (m >= 1) { L.a = take(ab); L.d0 = take(ab); L.tmp = take(ab); }
-        if (P.var) L.k = take(ab);
+        if (P.var) { L.k = take(ab); L.fz = take(ab); L.fy = take(ab); L.fx = take(ab); }
     }
     s->staging = take(P.staging_bytes);
     s->partial = static_cast<double*>(take(P.partial_count * sizeof(double)));

@@ -27,6 +27,7 @@ struct CoarseOp {
     long long count;          // OP_ZERO: elements
     LevelGeom go, gi, gv;     // output level, input level, level of the last visit (D0_DOWN)
     Coef<T> cf;
+    Faces<T> kf;              // OP_RELAX, variable coefficient
     const T* p[5];
     T* q[3];
 };
@@ -42,7 +43,7 @@ __device__ __forceinline__ T ldg_(const T* p) { return CG ? __ldcg(p) : *p; }
 
 // (A v)(c), D(c): homg_kernels.cuh node_A, with L2 loads
 template <class T, int ND, bool VAR, bool CG>
-__device__ __forceinline__ void cnode_A(const T* v, const T* k, long long c, const LevelGeom& g, const Coef<T>& cf,
+__device__ __forceinline__ void cnode_A(const T* v, const Faces<T>& kf, long long c, const LevelGeom& g, const Coef<T>& cf,
                                         T vc, T& Av, T& D) {
     if (!VAR) {
         T s = T(0);
@@ -52,18 +53,14 @@ __device__ __forceinline__ void cnode_A(const T* v, const T* k, long long c, con
         Av = (cf.twod * vc - s) * cf.ih2;
         D = cf.twod * cf.ih2;
     } else {
-        T kc = ldcg(k + c);
         T acc = T(0), dsum = T(0);
-        long long off[3] = {g.pp, (long long)g.px, 1};
+        const long long off[3] = {g.pp, (long long)g.px, 1};
+        const T* fa[3] = {kf.z, kf.y, kf.x};                 // written once at set_coefficient: plain loads
 #pragma unroll
         for (int a = 3 - ND; a < 3; ++a) {
-#pragma unroll
-            for (int sg = -1; sg <= 1; sg += 2) {
-                long long q = c + sg * off[a];
-                T kf = kface(kc, ldcg(k + q));
-                acc += kf * (vc - ldcg(v + q));
-                dsum += kf;
-            }
+            const T fm = fa[a][c - off[a]], fp = fa[a][c];
+            acc += fm * (vc - ldcg(v + c - off[a])); dsum += fm;
+            acc += fp * (vc - ldcg(v + c + off[a])); dsum += fp;
         }
         Av = acc * cf.ih2;
         D = dsum * cf.ih2;
@@ -171,7 +168,7 @@ __device__ __forceinline__ void coarse_node(const CoarseOp<T>& o, int x, int y, 
             vn = jacobi_eq3(vc, s, ldcg(o.p[1] + c), o.cf);
         } else {
             T Av, D;
-            cnode_A<T, ND, VAR, CG>(o.p[0], o.p[2], c, g, o.cf, vc, Av, D);
+            cnode_A<T, ND, VAR, CG>(o.p[0], o.kf, c, g, o.cf, vc, Av, D);
             vn = vc + o.cf.w * (ldcg(o.p[1] + c) - Av) / D;
         }
         vout[c] = vn;

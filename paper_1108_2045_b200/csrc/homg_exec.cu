@@ -126,6 +126,11 @@ Coef<T> make_coef(const homg_solver* s, int m) {
 }
 
 template <class T>
+Faces<T> faces(const Level& L) {
+    return Faces<T>{static_cast<const T*>(L.fz), static_cast<const T*>(L.fy), static_cast<const T*>(L.fx)};
+}
+
+template <class T>
 T* rotp(Level& L, int i) { return i < 0 ? nullptr : static_cast<T*>(L.rot[i]); }
 
 
@@ -180,20 +185,18 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
     Coef<T> cf = make_coef<T>(s, t);
     if (tiled(s, t)) {
         using TL = Tile<T, ND>;
-        CUtensorMap tmv, tmg, tmk;
+        CUtensorMap tmv, tmg;
         bool ok = make_tmap<T, ND>(s, &tmv, vin, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1) &&
                   make_tmap<T, ND>(s, &tmg, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
-        if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, Lt.k, Lt.g, TL::VW, ND == 3 ? TL::TY + 2 : 1);
-        else tmk = tmv;
         if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
         int nch = 1;
         int mc = march_chunk<T, ND>(s, Lt.g, &nch);
         dim3 grid((Lt.g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (Lt.g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
         if (u && t == 0) vout = nullptr;              // e_0 is dead after u += e_0: do not write it
-        klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, tmk, Lt.g, cf, vout, a, a_assign,
+        klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, faces<T>(Lt), Lt.g, cf, vout, a, a_assign,
                                                                                       d0, v0, u, mc);
     } else {
-        klaunch(R, k_relax<T, ND, VAR>, grd(Lt.g), blk(), 0, Lt.g, cf, vin, (const T*)(R.g_override ? R.g_override : Lt.gsrc), (const T*)Lt.k, vout, a,
+        klaunch(R, k_relax<T, ND, VAR>, grd(Lt.g), blk(), 0, Lt.g, cf, vin, (const T*)(R.g_override ? R.g_override : Lt.gsrc), faces<T>(Lt), vout, a,
                                                             a_assign, d0, v0, u);
     }
 }
@@ -207,12 +210,10 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
     Level& Lt = s->L[t];
     Level& Lc = s->L[t + 1];
     using TL = FirstTile<T, ND>;
-    CUtensorMap tme, tma_, tmg, tmk;
+    CUtensorMap tme, tma_, tmg;
     bool ok = make_tmap<T, ND>(s, &tme, ec, Lc.g, TL::CW, ND == 3 ? TL::CROWS : 1) &&
               make_tmap<T, ND>(s, &tma_, ac, Lc.g, TL::CW, ND == 3 ? TL::CROWS : 1) &&
               make_tmap<T, ND>(s, &tmg, Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
-    if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, Lt.k, Lt.g, TL::FW, ND == 3 ? TL::TY + 2 : 1);
-    else tmk = tmg;
     if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
     const LevelGeom& g = Lt.g;
     const int NM = ND == 3 ? g.nz : g.ny;
@@ -227,7 +228,7 @@ void launch_relax_first(Rec& R, int t, const T* ec, const T* ac, T* vout, T* u) 
     int nch = (interior + mc - 1) / mc;
     dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
     klaunch(R, k_relax_first<T, ND, VAR>, grid, TL::NW * 32, first_smem_bytes<T, ND, VAR>(), 
-        tme, tma_, tmg, tmk, g, make_coef<T>(s, t), (u && t == 0) ? (T*)nullptr : vout, u, mc);
+        tme, tma_, tmg, faces<T>(Lt), g, make_coef<T>(s, t), (u && t == 0) ? (T*)nullptr : vout, u, mc);
 }
 
 
@@ -319,11 +320,9 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
     bool fused_restrict = false;
     if (tiled(s, 0)) {
         using TL = ResTile<T, ND>;
-        CUtensorMap tmu, tmf, tmk;
+        CUtensorMap tmu, tmf;
         bool ok = make_tmap<T, ND>(s, &tmu, R.u_override ? R.u_override : s->u, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1) &&
                   make_tmap<T, ND>(s, &tmf, s->f, L0.g, TL::SEG, ND == 3 ? TL::TY + 1 : 1);
-        if (VAR) ok = ok && make_tmap<T, ND>(s, &tmk, L0.k, L0.g, TL::UW, ND == 3 ? TL::TY + 3 : 1);
-        else tmk = tmu;
         if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return false; }
         fused_restrict = restrict1 && write_r && s->levels >= 2;
         const LevelGeom& g = L0.g;
@@ -340,7 +339,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         dim3 grid((g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
         n = int(grid.x * grid.y * grid.z);
         if (!R.plan) klaunch(R, k_res_tma<T, ND, VAR>, grid, TL::NW * 32, res_smem_bytes<T, ND, VAR>(), 
-            tmu, tmf, tmk, g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
+            tmu, tmf, faces<T>(L0), g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
             fused_restrict ? (T*)s->L[1].gsrc : nullptr, s->partial, mc);
         R.check(TAG_RESIDUAL0);
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
@@ -348,7 +347,7 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
     } else {
         dim3 g = grd(L0.g);
         if (!R.plan) klaunch(R, k_residual<T, ND, VAR>, g, blk(), 0, L0.g, make_coef<T>(s, 0), (const T*)(R.u_override ? R.u_override : s->u), (const T*)s->f,
-                                                       (const T*)L0.k, write_r ? (T*)L0.gsrc : nullptr, s->partial);
+                                                       faces<T>(L0), write_r ? (T*)L0.gsrc : nullptr, s->partial);
         R.check(TAG_RESIDUAL0);
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
         n = int(g.x * g.y * g.z);
@@ -602,7 +601,7 @@ void rec_cycle(Rec& R) {
             if (small(t)) {
                 CoarseOp<T> o = newop(OP_RELAX, t);
                 o.cf = make_coef<T>(s, t);
-                o.p[0] = rotp<T>(Lt, in); o.p[1] = (const T*)Lt.gsrc; o.p[2] = (const T*)Lt.k;
+                o.p[0] = rotp<T>(Lt, in); o.p[1] = (const T*)Lt.gsrc; o.p[2] = nullptr; o.kf = faces<T>(Lt);
                 o.p[3] = have_d0 ? (const T*)Lt.d0 : nullptr; o.p[4] = rotp<T>(Lt, v0);
                 o.q[0] = rotp<T>(Lt, out); o.q[1] = book ? (T*)Lt.a : nullptr; o.q[2] = addu ? (T*)s->u : nullptr;
                 o.f0 = a_zero[t] ? 1 : 0;
@@ -697,7 +696,7 @@ void rec_vcycle(Rec& R) {
             }
         } else {
             klaunch(R, k_residual<T, ND, VAR>, grd(Lm.g), blk(), 0, Lm.g, make_coef<T>(s, m), (const T*)cur[m],
-                    (const T*)Lm.gsrc, (const T*)Lm.k, (T*)Lm.tmp, s->partial);
+                    (const T*)Lm.gsrc, faces<T>(Lm), (T*)Lm.tmp, s->partial);
             R.check(TAG_OTHER);
             R.acct(m, 3.0 + (VAR ? 1.0 : 0.0), TAG_OTHER);
             klaunch(R, k_restrict<T, ND>, grd(L[m + 1].g), blk(), 0, L[m + 1].g, Lm.g, (const T*)Lm.tmp, (T*)L[m + 1].gsrc);
@@ -711,7 +710,7 @@ void rec_vcycle(Rec& R) {
         cudaMemsetAsync(cur[M], 0, L[M].n_alloc * sizeof(T), R.st);
         R.check(TAG_OTHER);
         klaunch(R, k_coarsest_solve<T, ND, VAR>, dim3(1), dim3(32), 0, L[M].g, make_coef<T>(s, M), (const T*)L[M].gsrc,
-                (const T*)L[M].k, cur[M]);
+                faces<T>(L[M]), cur[M]);
         R.check(TAG_COARSE);
     }
     for (int m = M - 1; m >= 0; --m) {
@@ -736,6 +735,11 @@ void rec_sample(Rec& R) {
     for (int m = 1; m < s->levels; ++m) {
         klaunch(R, k_sample_coef<T, ND>, grd(s->L[m].g), blk(), 0, s->L[m].g, s->L[m - 1].g, (const T*)s->L[m - 1].k,
                                                                    (T*)s->L[m].k);
+        R.check(TAG_OTHER);
+    }
+    for (int m = 0; m < s->levels; ++m) {               // S0: face coefficients of every level
+        Level& Lm = s->L[m];
+        klaunch(R, k_faces<T, ND>, grd(Lm.g), blk(), 0, Lm.g, (const T*)Lm.k, (T*)Lm.fz, (T*)Lm.fy, (T*)Lm.fx);
         R.check(TAG_OTHER);
     }
 }

@@ -32,8 +32,6 @@ struct FirstTile {
     static constexpr int FROWS = ND == 3 ? TY + 2 : WX;
     static constexpr int FRS = ND == 3 ? FW : ((FW * ES + 127) / 128 * 128) / ES;
     static constexpr int FPLANE = FROWS * FRS;                       // elements
-    static constexpr int KBOX_BYTES = FROWS * FW * ES;
-    static constexpr int KTILE_BYTES = (FPLANE * ES + 127) / 128 * 128;
     static constexpr int NF = 4;                                     // fine ring slots
     // coarse tiles of e_c and a_c
     // TMA needs the box to START on a 16-B boundary of the row: the box begins at the coarse column
@@ -51,7 +49,7 @@ struct FirstTile {
 };
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int first_gk_stage_bytes() {
-    return FirstTile<T, ND>::GBOX_BYTES + (VAR ? FirstTile<T, ND>::KTILE_BYTES : 0);
+    return FirstTile<T, ND>::GBOX_BYTES;
 }
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int first_smem_bytes() {
@@ -61,12 +59,12 @@ __host__ __device__ constexpr int first_smem_bytes() {
 }
 
 
-// tme / tma_ : tensor maps of e_c and a_c (level c = f+1);  tmg / tmk : g_f and k_f (VAR).
+// tme / tma_ : tensor maps of e_c and a_c (level c = f+1);  tmg : g_f;  kf : face coefficients (VAR).
 // vout = v1;  u != null: u += v1 (a visit of a single sweep that ends the cycle).  mchunk even.
 template <class T, int ND, bool VAR>
 __global__ void __launch_bounds__(FirstTile<T, ND>::NW * 32)
 k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ CUtensorMap tma_,
-              const __grid_constant__ CUtensorMap tmg, const __grid_constant__ CUtensorMap tmk, LevelGeom g,
+              const __grid_constant__ CUtensorMap tmg, Faces<T> kf, LevelGeom g,
               Coef<T> cf, T* __restrict__ vout, T* __restrict__ u, int mchunk) {
     pdl_start();
     using TL = FirstTile<T, ND>;
@@ -90,7 +88,6 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
     unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
     __shared__ uint64_t fbar[TL::NG], cbar[TL::NC];
     auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * GK); };
-    auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * GK + TL::GBOX_BYTES); };
     unsigned char* cbase = smem + TL::NG * GK;
     auto ce = [&](int st) { return reinterpret_cast<T*>(cbase + (2 * st) * TL::CTILE_BYTES); };
     auto ca = [&](int st) { return reinterpret_cast<T*>(cbase + (2 * st + 1) * TL::CTILE_BYTES); };
@@ -106,16 +103,14 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
     auto issue_f = [&](int q) {                 // g and k of fine plane q
         const int st = q & (TL::NG - 1), p = ms - 1 + q;
         const bool wantg = q >= 1 && q <= nq - 2;
-        const uint32_t bytes = (wantg ? TL::GBOX_BYTES : 0) + (VAR ? TL::KBOX_BYTES : 0);
+        const uint32_t bytes = wantg ? TL::GBOX_BYTES : 0;
         if (bytes == 0) { mbar_arrive_expect_tx(&fbar[st], 0); return; }   // keeps the phase count = q / NG
         mbar_arrive_expect_tx(&fbar[st], bytes);
         if (ND == 3) {
             if (wantg) tma_load_3d(gs(st), &tmg, &fbar[st], x0 - VEC, y0, p);
-            if (VAR) tma_load_3d(ks(st), &tmk, &fbar[st], x0 - VEC, y0 - 1, p);
         } else {
             for (int w = 0; w < TL::WX; ++w) {
                 if (wantg) tma_load_2d(gs(st) + w * TL::SEG, &tmg, &fbar[st], x0 + w * TL::OWN - VEC, p);
-                if (VAR) tma_load_2d(ks(st) + w * TL::FRS, &tmk, &fbar[st], x0 + w * TL::OWN - VEC, p);
             }
         }
     };
@@ -204,19 +199,17 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
 
     produce(0);
     if (nq > 1) produce(1);
-    Pack<T> prv, cur, nxt, kprv, kcur, knxt;
-    if (VAR) {
-        mbar_wait(&fbar[0], 0);
-        kprv = *reinterpret_cast<const Pack<T>*>(ks(0) + foff);
-        mbar_wait(&fbar[1], 0);
-        kcur = *reinterpret_cast<const Pack<T>*>(ks(1) + foff);
-    }
+    Pack<T> prv, cur, nxt;
     __syncthreads();
     prv = *reinterpret_cast<const Pack<T>*>(fring + foff);
     cur = *reinterpret_cast<const Pack<T>*>(fring + TL::FPLANE + foff);
     if (tid == 0 && TL::NC < ncz) issue_c(TL::NC);
 
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
+    // VAR: face coefficients straight from global memory (see k_relax_tma)
+    const bool kok = VAR && relaxer && x >= 0 && x < g.nx && row_int;
+    Pack<T> fzm;
+    if (kok) fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
     auto step = [&](auto KC, const int q) {
         constexpr int K = decltype(KC)::value;              // (q-1) mod 4
         constexpr int sc = (K + 1) & 3, sn = (K + 2) & 3;    // ring slots of planes q and q+1
@@ -228,25 +221,25 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
             if ((K & 1) && (q >> 1) + TL::NC < ncz) issue_c((q >> 1) + TL::NC);
         }
         if (relaxer) {
-            if (VAR) mbar_wait(&fbar[sn], ((q + 1) / TL::NG) & 1);
-            else mbar_wait(&fbar[sc], (q / TL::NG) & 1);
+            Pack<T> fzp, fym, fyp, fxp;
+            T fxl = T(0);
+            if (kok) {
+                fzp = *reinterpret_cast<const Pack<T>*>(kf.z + c);
+                fym = *reinterpret_cast<const Pack<T>*>(kf.y + c - g.px);
+                fyp = *reinterpret_cast<const Pack<T>*>(kf.y + c);
+                fxp = *reinterpret_cast<const Pack<T>*>(kf.x + c);
+                if (x > 0) fxl = kf.x[c - 1];
+            }
+            mbar_wait(&fbar[sc], (q / TL::NG) & 1);
             const T* vn = fring + sn * TL::FPLANE;
             const T* vt = fring + sc * TL::FPLANE;
-            const T* kt = ks(sc);
             nxt = *reinterpret_cast<const Pack<T>*>(vn + foff);
-            if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + foff);
-            Pack<T> dn, up, kdn, kup;
+            Pack<T> dn, up;
             if (ND == 3) {
                 dn = *reinterpret_cast<const Pack<T>*>(vt + foff - TL::FRS);
                 up = *reinterpret_cast<const Pack<T>*>(vt + foff + TL::FRS);
-                if (VAR) {
-                    kdn = *reinterpret_cast<const Pack<T>*>(kt + foff - TL::FRS);
-                    kup = *reinterpret_cast<const Pack<T>*>(kt + foff + TL::FRS);
-                }
             }
             const T vl = vt[foff - 1], vr = vt[foff + VEC];
-            T kl = T(0), kr = T(0);
-            if (VAR) { kl = kt[foff - 1]; kr = kt[foff + VEC]; }
             const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs(sc) + goff);
             Pack<T> out;
 #pragma unroll
@@ -261,18 +254,16 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
                     s += xm + xp;
                     eq3 = jacobi_eq3(vc, s, gv.v[j], cf);
                 } else {
-                    const T kc = kcur.v[j];
-                    const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
-                    const T kxp = j == VEC - 1 ? kr : kcur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-                    T acc = T(0), ds = T(0), kf;
-                    kf = kface(kc, kprv.v[j]); acc += kf * (vc - prv.v[j]); ds += kf;
-                    kf = kface(kc, knxt.v[j]); acc += kf * (vc - nxt.v[j]); ds += kf;
+                    const T fxm = j == 0 ? fxl : fxp.v[j - 1 < 0 ? 0 : j - 1];
+                    T acc = T(0), ds = T(0);
+                    acc += fzm.v[j] * (vc - prv.v[j]); ds += fzm.v[j];
+                    acc += fzp.v[j] * (vc - nxt.v[j]); ds += fzp.v[j];
                     if (ND == 3) {
-                        kf = kface(kc, kdn.v[j]); acc += kf * (vc - dn.v[j]); ds += kf;
-                        kf = kface(kc, kup.v[j]); acc += kf * (vc - up.v[j]); ds += kf;
+                        acc += fym.v[j] * (vc - dn.v[j]); ds += fym.v[j];
+                        acc += fyp.v[j] * (vc - up.v[j]); ds += fyp.v[j];
                     }
-                    kf = kface(kc, kxm); acc += kf * (vc - xm); ds += kf;
-                    kf = kface(kc, kxp); acc += kf * (vc - xp); ds += kf;
+                    acc += fxm * (vc - xm); ds += fxm;
+                    acc += fxp.v[j] * (vc - xp); ds += fxp.v[j];
                     Av = acc * cf.ih2;
                     D = ds * cf.ih2;
                 }
@@ -288,7 +279,7 @@ k_relax_first(const __grid_constant__ CUtensorMap tme, const __grid_constant__ C
                 }
             }
             prv = cur; cur = nxt;
-            if (VAR) { kprv = kcur; kcur = knxt; }
+            if (VAR) fzm = fzp;
         }
         c += mstride;
     };

@@ -61,7 +61,7 @@ struct Tile {
 
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int relax_stage_bytes() {
-    return Tile<T, ND>::VTILE_BYTES * (VAR ? 2 : 1) + Tile<T, ND>::GBOX_BYTES;
+    return Tile<T, ND>::VTILE_BYTES + Tile<T, ND>::GBOX_BYTES;
 }
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int relax_smem_bytes() {
@@ -69,7 +69,8 @@ __host__ __device__ constexpr int relax_smem_bytes() {
 }
 
 // S3d (+S3e, +S4): one damped-Jacobi sweep  vout = vin + w (g - A vin)/D  on a large level.
-//   tmv / tmk / tmg : tensor maps of vin, k (VAR) and g of this level
+//   tmv / tmg : tensor maps of vin and g of this level;  kf : face coefficients (VAR), read straight
+//   from global memory as coalesced 16-byte packs (own pack of fz / fy / fx, the y-1 row of fy, one scalar of fx)
 //   a, a_assign, d0, v0, u : the optional epilogues of k_relax (same meaning)
 //   vout may be null when u is given (last sweep of the cycle: e_0 is dead after u += e_0)
 //   mchunk : interior planes per CTA along the marching axis
@@ -77,7 +78,7 @@ __host__ __device__ constexpr int relax_smem_bytes() {
 template <class T, int ND, bool VAR>
 __global__ void __launch_bounds__(256)
 k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUtensorMap tmg,
-            const __grid_constant__ CUtensorMap tmk, LevelGeom g, Coef<T> cf, T* __restrict__ vout,
+            Faces<T> kf, LevelGeom g, Coef<T> cf, T* __restrict__ vout,
             T* __restrict__ a, int a_assign, const T* __restrict__ d0, const T* __restrict__ v0,
             T* __restrict__ u, int mchunk) {
     pdl_start();
@@ -100,8 +101,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // keeps the shared address space
     __shared__ uint64_t bars[TL::NST];
     auto vs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
-    auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES); };
-    auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES * (VAR ? 2 : 1)); };
+    auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::VTILE_BYTES); };
 
     if (tid == 0) {
         for (int s = 0; s < TL::NST; ++s) mbar_init(&bars[s], 1);
@@ -112,10 +112,9 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     auto issue = [&](int i) {                            // relative plane i = absolute ms-1+i
         const int st = i & (TL::NST - 1), p = ms - 1 + i;
         const bool wantg = i >= 1 && i <= count - 2;
-        mbar_arrive_expect_tx(&bars[st], TL::VBOX_BYTES * (VAR ? 2 : 1) + (wantg ? TL::GBOX_BYTES : 0));
+        mbar_arrive_expect_tx(&bars[st], TL::VBOX_BYTES + (wantg ? TL::GBOX_BYTES : 0));
         if (ND == 3) {
             tma_load_3d(vs(st), &tmv, &bars[st], x0 - VEC, y0 - 1, p);
-            if (VAR) tma_load_3d(ks(st), &tmk, &bars[st], x0 - VEC, y0 - 1, p);
             if (wantg) tma_load_3d(gs(st), &tmg, &bars[st], x0, y0, p);
         } else {
             for (int w = 0; w < TL::WX; ++w) {
@@ -140,38 +139,41 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     if (tid == 0)
         for (int i = 0; i < TL::NST && i < count; ++i) issue(i);
 
-    Pack<T> prv, cur, nxt, kprv, kcur, knxt;
+    Pack<T> prv, cur, nxt;
     mbar_wait(&bars[0], 0);
     prv = *reinterpret_cast<const Pack<T>*>(vs(0) + voff);
-    if (VAR) kprv = *reinterpret_cast<const Pack<T>*>(ks(0) + voff);
     mbar_wait(&bars[1], 0);
     cur = *reinterpret_cast<const Pack<T>*>(vs(1) + voff);
-    if (VAR) kcur = *reinterpret_cast<const Pack<T>*>(ks(1) + voff);
     __syncthreads();
     if (tid == 0 && TL::NST < count) issue(TL::NST);
 
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
+    // VAR: faces of this thread's nodes; the z- face of a plane is the z+ face of the one before
+    const bool kok = VAR && row_ok && row_int;
+    Pack<T> fzm;
+    if (kok) fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
     // one plane; K = (i-1) mod 4 is a compile-time constant so that every stage address is an immediate
     auto step = [&](auto KC, const int i) {
         constexpr int K = decltype(KC)::value;
         constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
+        Pack<T> fzp, fym, fyp, fxp;
+        T fxl = T(0);
+        if (kok) {
+            fzp = *reinterpret_cast<const Pack<T>*>(kf.z + c);
+            fym = *reinterpret_cast<const Pack<T>*>(kf.y + c - g.px);
+            fyp = *reinterpret_cast<const Pack<T>*>(kf.y + c);
+            fxp = *reinterpret_cast<const Pack<T>*>(kf.x + c);
+            if (x > 0) fxl = kf.x[c - 1];
+        }
         nxt = *reinterpret_cast<const Pack<T>*>(vs(sn) + voff);
-        if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
         const T* vt = vs(sc);
-        const T* kt = ks(sc);
-        Pack<T> dn, up, kdn, kup;
+        Pack<T> dn, up;
         if (ND == 3) {
             dn = *reinterpret_cast<const Pack<T>*>(vt + voff - TL::VRS);
             up = *reinterpret_cast<const Pack<T>*>(vt + voff + TL::VRS);
-            if (VAR) {
-                kdn = *reinterpret_cast<const Pack<T>*>(kt + voff - TL::VRS);
-                kup = *reinterpret_cast<const Pack<T>*>(kt + voff + TL::VRS);
-            }
         }
         const T vl = vt[voff - 1], vr = vt[voff + VEC];
-        T kl = T(0), kr = T(0);
-        if (VAR) { kl = kt[voff - 1]; kr = kt[voff + VEC]; }
         const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs(sc) + goff);
         Pack<T> out;
 #pragma unroll
@@ -186,18 +188,16 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
                 s += xm + xp;
                 eq3 = jacobi_eq3(vc, s, gv.v[j], cf);
             } else {
-                const T kc = kcur.v[j];
-                const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
-                const T kxp = j == VEC - 1 ? kr : kcur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-                T acc = T(0), ds = T(0), kf;
-                kf = kface(kc, kprv.v[j]); acc += kf * (vc - prv.v[j]); ds += kf;
-                kf = kface(kc, knxt.v[j]); acc += kf * (vc - nxt.v[j]); ds += kf;
+                const T fxm = j == 0 ? fxl : fxp.v[j - 1 < 0 ? 0 : j - 1];
+                T acc = T(0), ds = T(0);
+                acc += fzm.v[j] * (vc - prv.v[j]); ds += fzm.v[j];
+                acc += fzp.v[j] * (vc - nxt.v[j]); ds += fzp.v[j];
                 if (ND == 3) {
-                    kf = kface(kc, kdn.v[j]); acc += kf * (vc - dn.v[j]); ds += kf;
-                    kf = kface(kc, kup.v[j]); acc += kf * (vc - up.v[j]); ds += kf;
+                    acc += fym.v[j] * (vc - dn.v[j]); ds += fym.v[j];
+                    acc += fyp.v[j] * (vc - up.v[j]); ds += fyp.v[j];
                 }
-                kf = kface(kc, kxm); acc += kf * (vc - xm); ds += kf;
-                kf = kface(kc, kxp); acc += kf * (vc - xp); ds += kf;
+                acc += fxm * (vc - xm); ds += fxm;
+                acc += fxp.v[j] * (vc - xp); ds += fxp.v[j];
                 Av = acc * cf.ih2;
                 D = ds * cf.ih2;
             }
@@ -226,7 +226,7 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
         __syncthreads();
         if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
         prv = cur; cur = nxt;
-        if (VAR) { kprv = kcur; kcur = knxt; }
+        if (VAR) fzm = fzp;
         c += mstride;
     };
     for (int i = 1; i <= count - 2; i += 4) {
@@ -274,7 +274,7 @@ struct ResTile {
 };
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int res_stage_bytes() {
-    return ResTile<T, ND>::UTILE_BYTES * (VAR ? 2 : 1) + ResTile<T, ND>::FBOX_BYTES;
+    return ResTile<T, ND>::UTILE_BYTES + ResTile<T, ND>::FBOX_BYTES;
 }
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int res_smem_bytes() {
@@ -285,7 +285,7 @@ __host__ __device__ constexpr int res_smem_bytes() {
 template <class T, int ND, bool VAR>
 __global__ void __launch_bounds__(ResTile<T, ND>::NW * 32)
 k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUtensorMap tmf,
-          const __grid_constant__ CUtensorMap tmk, LevelGeom g, LevelGeom gcg, Coef<T> cf, T* __restrict__ r,
+          Faces<T> kf, LevelGeom g, LevelGeom gcg, Coef<T> cf, T* __restrict__ r,
           T* __restrict__ gc, double* __restrict__ partial, int mchunk) {
     pdl_start();
     using TL = ResTile<T, ND>;
@@ -310,8 +310,7 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // keeps the shared address space
     __shared__ uint64_t bars[TL::NST];
     auto us = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE); };
-    auto ks = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES); };
-    auto fs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES * (VAR ? 2 : 1)); };
+    auto fs = [&](int st) { return reinterpret_cast<T*>(smem + st * STAGE + TL::UTILE_BYTES); };
     T* rring = reinterpret_cast<T*>(smem + TL::NST * STAGE);
 
     if (tid == 0) {
@@ -323,10 +322,9 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     auto issue = [&](int i) {
         const int st = i & (TL::NST - 1), p = ms - 1 + i;
         const bool wantf = i >= 1 && i <= count - 2;
-        mbar_arrive_expect_tx(&bars[st], TL::UBOX_BYTES * (VAR ? 2 : 1) + (wantf ? TL::FBOX_BYTES : 0));
+        mbar_arrive_expect_tx(&bars[st], TL::UBOX_BYTES + (wantf ? TL::FBOX_BYTES : 0));
         if (ND == 3) {
             tma_load_3d(us(st), &tmu, &bars[st], x0 - 2 * VEC, y0 - 2, p);
-            if (VAR) tma_load_3d(ks(st), &tmk, &bars[st], x0 - 2 * VEC, y0 - 2, p);
             if (wantf) tma_load_3d(fs(st), &tmf, &bars[st], x0 - VEC, y0 - 1, p);
         } else {
             for (int w = 0; w < TL::WX; ++w) {
@@ -351,39 +349,42 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     if (tid == 0)
         for (int i = 0; i < TL::NST && i < count; ++i) issue(i);
 
-    Pack<T> prv, cur, nxt, kprv, kcur, knxt;
+    Pack<T> prv, cur, nxt;
     mbar_wait(&bars[0], 0);
     prv = *reinterpret_cast<const Pack<T>*>(us(0) + voff);
-    if (VAR) kprv = *reinterpret_cast<const Pack<T>*>(ks(0) + voff);
     mbar_wait(&bars[1], 0);
     cur = *reinterpret_cast<const Pack<T>*>(us(1) + voff);
-    if (VAR) kcur = *reinterpret_cast<const Pack<T>*>(ks(1) + voff);
     __syncthreads();
     if (tid == 0 && TL::NST < count) issue(TL::NST);
 
     double sq = 0.0;
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
+    // VAR: face coefficients straight from global memory (see k_relax_tma)
+    const bool kok = VAR && x >= 0 && x < g.nx && row_int;
+    Pack<T> fzm;
+    if (kok) fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
     auto step = [&](auto KC, const int i) {
         constexpr int K = decltype(KC)::value;
         const int z = ms - 1 + i;
         constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
+        Pack<T> fzp, fym, fyp, fxp;
+        T fxl = T(0);
+        if (kok) {
+            fzp = *reinterpret_cast<const Pack<T>*>(kf.z + c);
+            fym = *reinterpret_cast<const Pack<T>*>(kf.y + c - g.px);
+            fyp = *reinterpret_cast<const Pack<T>*>(kf.y + c);
+            fxp = *reinterpret_cast<const Pack<T>*>(kf.x + c);
+            if (x > 0) fxl = kf.x[c - 1];
+        }
         nxt = *reinterpret_cast<const Pack<T>*>(us(sn) + voff);
-        if (VAR) knxt = *reinterpret_cast<const Pack<T>*>(ks(sn) + voff);
         const T* vt = us(sc);
-        const T* kt = ks(sc);
-        Pack<T> dn, up, kdn, kup;
+        Pack<T> dn, up;
         if (ND == 3) {
             dn = *reinterpret_cast<const Pack<T>*>(vt + voff - TL::URS);
             up = *reinterpret_cast<const Pack<T>*>(vt + voff + TL::URS);
-            if (VAR) {
-                kdn = *reinterpret_cast<const Pack<T>*>(kt + voff - TL::URS);
-                kup = *reinterpret_cast<const Pack<T>*>(kt + voff + TL::URS);
-            }
         }
         const T vl = vt[voff - 1], vr = vt[voff + VEC];
-        T kl = T(0), kr = T(0);
-        if (VAR) { kl = kt[voff - 1]; kr = kt[voff + VEC]; }
         const Pack<T> fv = *reinterpret_cast<const Pack<T>*>(fs(sc) + foff);
         Pack<T> out;
 #pragma unroll
@@ -398,18 +399,16 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
                 s += xm + xp;
                 Av = (cf.twod * vc - s) * cf.ih2;
             } else {
-                const T kc = kcur.v[j];
-                const T kxm = j == 0 ? kl : kcur.v[j - 1 < 0 ? 0 : j - 1];
-                const T kxp = j == VEC - 1 ? kr : kcur.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+                const T fxm = j == 0 ? fxl : fxp.v[j - 1 < 0 ? 0 : j - 1];
                 T acc = T(0);
-                acc += kface(kc, kprv.v[j]) * (vc - prv.v[j]);
-                acc += kface(kc, knxt.v[j]) * (vc - nxt.v[j]);
+                acc += fzm.v[j] * (vc - prv.v[j]);
+                acc += fzp.v[j] * (vc - nxt.v[j]);
                 if (ND == 3) {
-                    acc += kface(kc, kdn.v[j]) * (vc - dn.v[j]);
-                    acc += kface(kc, kup.v[j]) * (vc - up.v[j]);
+                    acc += fym.v[j] * (vc - dn.v[j]);
+                    acc += fyp.v[j] * (vc - up.v[j]);
                 }
-                acc += kface(kc, kxm) * (vc - xm);
-                acc += kface(kc, kxp) * (vc - xp);
+                acc += fxm * (vc - xm);
+                acc += fxp.v[j] * (vc - xp);
                 Av = acc * cf.ih2;
             }
             out.v[j] = xin[j] ? fv.v[j] - Av : T(0);
@@ -423,7 +422,7 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
         __syncthreads();
         if (tid == 0 && i + TL::NST < count) issue(i + TL::NST);
         prv = cur; cur = nxt;
-        if (VAR) { kprv = kcur; kcur = knxt; }
+        if (VAR) fzm = fzp;
         c += mstride;
         if ((K & 1) == 0 && gc != nullptr && i >= 3) {
             // coarse plane Z = (z-1)/2 from r planes z-2, z-1, z (ring slots i-2, i-1, i)

@@ -9,6 +9,17 @@ struct LevelGeom {
     long long pp;        // plane pitch in elements (px*ny)
 };
 
+// Variable-coefficient stencil (R11): harmonic-mean face coefficients, precomputed per level at
+// homg_set_coefficient (S0).  z[c] / y[c] / x[c] = 2 k_c k_q / (k_c + k_q) for the face between node c and
+// its +z / +y / +x neighbour q (0 where q does not exist).  The face value is symmetric in (c, q), so
+// both nodes of a face read the very number the oracle computes from either side.
+template <class T>
+struct Faces {
+    const T* z;
+    const T* y;
+    const T* x;
+};
+
 template <class T>
 struct Coef {            // per-level operator constants
     T ih2;               // 1/h_m^2

@@ -29,6 +29,9 @@ struct Level {
     void* d0 = nullptr;        // carried variation (levels >= 1)
     void* tmp = nullptr;       // scratch of the d0 prolongation chain (levels >= 1)
     void* k = nullptr;         // nodal coefficient (HOMG_DIFFUSION7)
+    void* fz = nullptr;        // face coefficients towards +z / +y / +x (HOMG_DIFFUSION7; homg_geom.h Faces)
+    void* fy = nullptr;
+    void* fx = nullptr;
     // --- executor state while one cycle is being recorded ---
     int e = 0;                 // rot index holding the materialised correction e_m
     bool touched = false;      // e_m / a_m already defined in this cycle

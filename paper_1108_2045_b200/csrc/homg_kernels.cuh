@@ -44,7 +44,7 @@ __device__ __forceinline__ T kface(T kc, T kq) { return T(2) * kc * kq / (kc + k
 // (2d v - sum_nb v)/h^2, D = 2d/h^2.  Variable: sum_faces kf (v_c - v_q)/h^2, D = sum kf/h^2.
 // Neighbour order: slowest axis first (z, y, x), minus then plus (Eq.3).
 template <class T, int ND, bool VAR>
-__device__ __forceinline__ void node_A(const T* __restrict__ v, const T* __restrict__ k, long long c,
+__device__ __forceinline__ void node_A(const T* __restrict__ v, const Faces<T>& kf, long long c,
                                        const LevelGeom& g, const Coef<T>& cf, T& Av, T& D) {
     if (!VAR) {
         T s = T(0);
@@ -54,18 +54,15 @@ __device__ __forceinline__ void node_A(const T* __restrict__ v, const T* __restr
         Av = (cf.twod * v[c] - s) * cf.ih2;
         D = cf.twod * cf.ih2;
     } else {
-        T kc = k[c], vc = v[c];
+        const T vc = v[c];
         T acc = T(0), dsum = T(0);
-        long long off[3] = {g.pp, (long long)g.px, 1};
+        const long long off[3] = {g.pp, (long long)g.px, 1};
+        const T* fa[3] = {kf.z, kf.y, kf.x};
 #pragma unroll
         for (int a = 3 - ND; a < 3; ++a) {
-#pragma unroll
-            for (int sg = -1; sg <= 1; sg += 2) {
-                long long q = c + sg * off[a];
-                T kf = kface(kc, k[q]);
-                acc += kf * (vc - v[q]);
-                dsum += kf;
-            }
+            const T fm = fa[a][c - off[a]], fp = fa[a][c];       // faces towards the - and + neighbour
+            acc += fm * (vc - v[c - off[a]]); dsum += fm;
+            acc += fp * (vc - v[c + off[a]]); dsum += fp;
         }
         Av = acc * cf.ih2;
         D = dsum * cf.ih2;
@@ -88,7 +85,7 @@ __device__ __forceinline__ T jacobi_eq3(T vc, T s, T gval, const Coef<T>& cf) {
 
 // damped Jacobi at one interior node
 template <class T, int ND, bool VAR>
-__device__ __forceinline__ T node_jacobi(const T* __restrict__ v, const T* __restrict__ k, T gval,
+__device__ __forceinline__ T node_jacobi(const T* __restrict__ v, const Faces<T>& k, T gval,
                                          long long c, const LevelGeom& g, const Coef<T>& cf) {
     if (!VAR) {
         T s = T(0);
@@ -136,7 +133,7 @@ __device__ __forceinline__ double block_sum(double v) {
 // -> partial[linear block id].  r may be null (norm only).
 template <class T, int ND, bool VAR>
 __global__ void k_residual(LevelGeom g, Coef<T> cf, const T* __restrict__ u, const T* __restrict__ f,
-                           const T* __restrict__ k, T* __restrict__ r, double* __restrict__ partial) {
+                           Faces<T> k, T* __restrict__ r, double* __restrict__ partial) {
     pdl_start();
     int x = blockIdx.x * blockDim.x + threadIdx.x;
     int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -292,7 +289,7 @@ __global__ void k_d0_down(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, c
 // Boundary nodes are written too (with 0) so a buffer that held an older iterate is fully defined.
 template <class T, int ND, bool VAR>
 __global__ void k_relax(LevelGeom g, Coef<T> cf, const T* __restrict__ vin, const T* __restrict__ gsrc,
-                        const T* __restrict__ k, T* __restrict__ vout, T* __restrict__ a, int a_assign,
+                        Faces<T> k, T* __restrict__ vout, T* __restrict__ a, int a_assign,
                         const T* __restrict__ d0, const T* __restrict__ v0, T* __restrict__ u) {
     pdl_start();
     HOMG_NODE_XYZ(g);
@@ -327,6 +324,18 @@ __global__ void k_unpack(LevelGeom g, const T* __restrict__ padded, T* __restric
     pdl_start();
     HOMG_NODE_XYZ(g);
     dense[((long long)z * g.ny + y) * g.nx + x] = padded[lidx(g, x, y, z)];
+}
+
+// S0: face coefficients of one level from its nodal k (R11); 0 where the + neighbour does not exist
+template <class T, int ND>
+__global__ void k_faces(LevelGeom g, const T* __restrict__ k, T* __restrict__ fz, T* __restrict__ fy, T* __restrict__ fx) {
+    pdl_start();
+    HOMG_NODE_XYZ(g);
+    const long long c = lidx(g, x, y, z);
+    const T kc = k[c];
+    fx[c] = x + 1 < g.nx ? kface(kc, k[c + 1]) : T(0);
+    fy[c] = y + 1 < g.ny ? kface(kc, k[c + g.px]) : T(0);
+    if (ND == 3) fz[c] = z + 1 < g.nz ? kface(kc, k[c + g.pp]) : T(0);
 }
 
 // coefficient sampling onto the next level: k_c(P) = k_f(2P)     (R11)

@@ -43,8 +43,8 @@ bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, hom
         P.g.push_back(g);
         P.n_alloc.push_back(na);
         size_t arrays;
-        if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 1 : 0);
-        else arrays = kNumRot + 4 /*a g d0 tmp*/ + (P.var ? 1 : 0);
+        if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 4 : 0) /*k fz fy fx*/;
+        else arrays = kNumRot + 4 /*a g d0 tmp*/ + (P.var ? 4 : 0);
         total += arrays * na * es;
     }
     const LevelGeom& g0 = P.g[0];

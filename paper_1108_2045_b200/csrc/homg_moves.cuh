@@ -132,7 +132,7 @@ k_prolong_add_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, T* __restr
 // Classic V-cycle, step (c) on a coarsest level with ONE interior node (3^d grid): the exact solve
 // e = g / D, evaluated in double as the oracle's 1x1 LU does (D = the operator's diagonal in T).
 template <class T, int ND, bool VAR>
-__global__ void k_coarsest_solve(LevelGeom g, Coef<T> cf, const T* __restrict__ gsrc, const T* __restrict__ k,
+__global__ void k_coarsest_solve(LevelGeom g, Coef<T> cf, const T* __restrict__ gsrc, Faces<T> kf,
                                  T* __restrict__ e) {
     pdl_start();
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
@@ -141,13 +141,13 @@ __global__ void k_coarsest_solve(LevelGeom g, Coef<T> cf, const T* __restrict__ 
     if (!VAR) {
         D = cf.twod * cf.ih2;
     } else {
-        const T kc = k[c];
         T acc = T(0);
         const long long off[3] = {g.pp, (long long)g.px, 1};
+        const T* fa[3] = {kf.z, kf.y, kf.x};
 #pragma unroll
         for (int a = 3 - ND; a < 3; ++a) {
-            acc += kface(kc, k[c - off[a]]) * (T(1) - T(0));
-            acc += kface(kc, k[c + off[a]]) * (T(1) - T(0));
+            acc += fa[a][c - off[a]] * (T(1) - T(0));
+            acc += fa[a][c] * (T(1) - T(0));
         }
         D = acc * cf.ih2;
     }
