@@ -245,11 +245,12 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
 // K_res: fused residual + ||r||^2 partial + first full-weighting restriction (S1 + S2 first step + S5).
 //
 // The CTA computes r = f - A u on an r-tile that is one node wider than what it owns, on the low
-// side of every axis (full weighting of the coarse nodes of a tile needs r at 2I-1): 3-D: 9 warps,
-// warp R = fine row y0-1+R (row 0 is the recomputed halo row, rows 1..8 are owned); in every row
-// lane 0 holds the recomputed halo pack [xs-VEC, xs), lanes 1..31 the owned packs, so a tile owns
-// 31*VEC x 8 nodes per plane and every thread runs the same code.  2-D: 8 warps = 8 x-segments of
-// one row, each with its private halo pack.  The last four r planes stay in shared memory; after
+// side of every axis (full weighting of the coarse nodes of a tile needs r at 2I-1).  3-D: a row of
+// the r-tile is 33 packs: pack 0 is the recomputed halo pack [x0-VEC, x0), packs 1..32 are owned, so
+// a tile owns 32*VEC x 8 nodes per plane (power-of-two widths: 2^k+1 grids tile without a mostly
+// empty last tile).  Warps 0..8 = fine rows y0-1 .. y0+7 (row 0 is the recomputed halo row), lane l =
+// pack l+1; warp 9 computes the 9 halo packs (lane l = row l; its other lanes repeat row 0).  2-D: 8
+// warps = 8 x-segments of one row, lane 0 of each its private halo pack.  Every thread runs the same code.  The last four r planes stay in shared memory; after
 // an odd plane z = 2Z+1 the CTA writes the coarse plane Z (27 / 9 terms in the oracle's order).
 // A chunk [ms, me) of the marching axis (ms odd, even length) recomputes plane `me` for the same
 // reason.  r may be null (norm only); gc may be null (no restriction).
@@ -257,10 +258,11 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
 template <class T, int ND>
 struct ResTile {
     static constexpr int VEC = 16 / int(sizeof(T));
-    static constexpr int NW = ND == 3 ? 9 : 8;           // warps
+    static constexpr int NW = ND == 3 ? 10 : 8;          // warps
     static constexpr int WX = ND == 3 ? 1 : 8;           // x segments
-    static constexpr int SEG = 32 * VEC;                 // r nodes per warp row (halo pack + owned)
-    static constexpr int OWN = 31 * VEC;                 // owned x nodes per segment
+    static constexpr int NPK = ND == 3 ? 33 : 32;        // packs per row segment, halo pack included
+    static constexpr int SEG = NPK * VEC;                // r nodes per row segment (halo pack + owned)
+    static constexpr int OWN = (NPK - 1) * VEC;          // owned x nodes per segment
     static constexpr int TX = WX * OWN, TY = ND == 3 ? 8 : 1;
     static constexpr int UW = SEG + 2 * VEC;
     static constexpr int UROWS = ND == 3 ? TY + 3 : WX;
@@ -269,12 +271,13 @@ struct ResTile {
     static constexpr int UTILE_BYTES = (UROWS * URS * int(sizeof(T)) + 127) / 128 * 128;
     static constexpr int FROWS = ND == 3 ? TY + 1 : WX;
     static constexpr int FBOX_BYTES = FROWS * SEG * int(sizeof(T));
+    static constexpr int FTILE_BYTES = (FBOX_BYTES + 127) / 128 * 128;
     static constexpr int RPLANE = FROWS * SEG;           // elements of one r plane in shared memory
     static constexpr int NST = 4, NR = 4;
 };
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int res_stage_bytes() {
-    return ResTile<T, ND>::UTILE_BYTES + ResTile<T, ND>::FBOX_BYTES;
+    return ResTile<T, ND>::UTILE_BYTES + ResTile<T, ND>::FTILE_BYTES;
 }
 template <class T, int ND, bool VAR>
 __host__ __device__ constexpr int res_smem_bytes() {
@@ -291,7 +294,11 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     using TL = ResTile<T, ND>;
     constexpr int VEC = TL::VEC;
     constexpr int STAGE = res_stage_bytes<T, ND, VAR>();
-    const int tid = threadIdx.x, lane = tid & 31, R = tid >> 5;
+    const int tid = threadIdx.x;
+    // (row R, pack lane) of this thread inside the r-tile; "lane" 0 is the halo pack
+    const int wrp = tid >> 5, ln = tid & 31;
+    const int R = ND == 3 ? (wrp < 9 ? wrp : (ln < 9 ? ln : 0)) : wrp;
+    const int lane = ND == 3 ? (wrp < 9 ? ln + 1 : 0) : ln;
     const int NM = ND == 3 ? g.nz : g.ny;
     const long long mstride = ND == 3 ? g.pp : (long long)g.px;
     const int x0 = blockIdx.x * TL::TX;
