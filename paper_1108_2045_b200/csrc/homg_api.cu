@@ -109,6 +109,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (const char* ev = std::getenv("HOMG_MARCH_CHUNK")) s->march_chunk = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_PDL")) s->pdl = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
+    if (const char* ev = std::getenv("HOMG_FUSE_FIRST_VAR")) s->fuse_first_var = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     s->vcycle = o.cycle == HOMG_CYCLE_V;
     s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;

@@ -417,7 +417,7 @@ void rec_cycle(Rec& R) {
                     Level& Lc = L[m];
                     Level& Lf = L[m - 1];
                     int ef_assign = Lf.touched ? 0 : 1;
-                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && s->fuse_first) {
+                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && (VAR ? s->fuse_first_var : s->fuse_first)) {
                         fuse_first = true;                   // S3a of this hop happens inside the first sweep
                         fuse_ec = rotp<T>(Lc, Lc.e);
                         Lf.touched = true;

@@ -245,6 +245,11 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
         const bool fin = own && (STEADY || q >= 2 * NS);
         Pack<T> uu;
         if (fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
+        if (fin && a) {                                            // S3e operands: into L1 now (no registers), read after the stages
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(v0 + cF));
+            if (d0) asm volatile("prefetch.global.L1 [%0];" ::"l"(d0 + cF));
+            if (!a_assign) asm volatile("prefetch.global.L1 [%0];" ::"l"(a + cF));
+        }
         // stage s reads g of plane z0-s from the g ring; plane z0-1 is new in this step
         if (STEADY || q >= 1) mbar_wait(&gbar[(q - 1) & (TL::NGR - 1)], ((q - 1) / TL::NGR) & 1);
 #pragma unroll

@@ -220,6 +220,28 @@ def test_tiled_matches_generic_bitwise(orc):
         assert np.array_equal(x, y)
 
 
+@pytest.mark.parametrize("name,n,maxi", [("cfg4", 129, 4), ("cfg2", 65, 3), ("cfg3", 1025, 4), ("cfg4", 65, 8), ("cfg1", 513, 2)])
+def test_kvisit_matches_per_sweep_kernels_bitwise(orc, monkeypatch, name, n, maxi):
+    """K_visit (all sweeps of a visit in one pass, halo recompute, chunked marching axis) is bit-identical to
+    one launch per sweep, at sizes of several tiles with ragged tails, for NS = 2, 3, 4 and chunked visits."""
+    import dataclasses
+    cfg = dataclasses.replace(I.scaled(I.CONFIGS[name], n), max_iters=maxi)
+    inp = I.make_inputs(cfg)
+    a, na, _ = run_gpu(cfg, inp, 2)
+    monkeypatch.setenv("HOMG_FUSE_VISIT", "0")
+    b, nb, _ = run_gpu(cfg, inp, 2)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert np.array_equal(na, nb)
+
+
+def test_variable_coefficient_fused_first_sweep(orc, monkeypatch):
+    """k_relax_first for the variable-coefficient stencil (off by default: slower than deliver + sweep on cfg5)."""
+    monkeypatch.setenv("HOMG_FUSE_FIRST_VAR", "1")
+    check_parity(I.scaled(I.CONFIGS["cfg5"], 65), 3, orc)
+    check_parity(I.scaled(I.CONFIGS["cfg5"], 33), 3, orc, tiled_min_nodes=1, march_chunk=6)
+
+
 # ---- classic V(eta1, eta2) cycle on the GPU (PAPER.md L47; SURVEY.md 8(f)1) vs the oracle's Algorithm V ----
 def check_vcycle(cfg, ncycles, orc, eta=(2, 1), **kw):
     inp = I.make_inputs(cfg)
