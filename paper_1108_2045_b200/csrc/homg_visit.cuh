@@ -252,22 +252,38 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
         }
         // stage s reads g of plane z0-s from the g ring; plane z0-1 is new in this step
         if (STEADY || q >= 1) mbar_wait(&gbar[(q - 1) & (TL::NGR - 1)], ((q - 1) / TL::NGR) & 1);
-#pragma unroll
-        for (int s = 1; s <= NS; ++s) {
-            // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
+        // shared-memory operands of a stage (y neighbours, g; 2-D: the x neighbours across warp borders).
+        // They were published in the previous step, so the operands of stage s+1 are fetched BEFORE stage s
+        // computes and stores: the compiler cannot move a load above a shared store by itself.
+        auto fetch = [&](const int s, Pack<T>& dn, Pack<T>& up, Pack<T>& gv, T& el, T& er) {
             const T* ctr = (s == 1 && !INTERP) ? vring(SC) : buf(s - 1, R);
-            Pack<T> dn, up;
             if (ND == 3) {
                 dn = *reinterpret_cast<const Pack<T>*>(ctr + off - RS);
                 up = *reinterpret_cast<const Pack<T>*>(ctr + off + RS);
+            } else {
+                if ((tid & 31) == 0) el = ctr[off - 1];
+                if ((tid & 31) == 31) er = ctr[off + VEC];
             }
+            gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
+        };
+        // (3-D: one CTA of 512 threads per SM leaves 128 registers per thread; fetching ahead spills there)
+        constexpr bool AHEAD = ND == 2;
+        Pack<T> dnN, upN, gvN;
+        T elN = T(0), erN = T(0);
+        if (AHEAD) fetch(1, dnN, upN, gvN, elN, erN);
+#pragma unroll
+        for (int s = 1; s <= NS; ++s) {
+            // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
+            if (!AHEAD) fetch(s, dnN, upN, gvN, elN, erN);
+            const Pack<T> dn = dnN, up = upN, gv = gvN;
+            const T el = elN, er = erN;
+            if (AHEAD && s < NS) fetch(s + 1, dnN, upN, gvN, elN, erN);
             const Pack<T> cu = C[s - 1], pv = P[s - 1];
-            const Pack<T> gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
             T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
             T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
             if (ND == 2) {                                         // a row spans several warps
-                if ((tid & 31) == 0) vl = ctr[off - 1];
-                if ((tid & 31) == 31) vr = ctr[off + VEC];
+                if ((tid & 31) == 0) vl = el;
+                if ((tid & 31) == 31) vr = er;
             }
             const int z = z0 - s;
             const bool zin = STEADY || (z > 0 && z < NM - 1);
