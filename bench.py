@@ -40,8 +40,9 @@ def parse():
     ap.add_argument("--impl", default="homg", choices=["homg", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=sorted(I.CONFIGS))
     ap.add_argument("--n", type=int, default=0, help="scale the workload to an n^d grid (debugging)")
-    ap.add_argument("--cycle", default="mfmg", choices=["mfmg", "v"],
-                    help="mfmg: the paper's HOMG cycle (default); v: classic V(2,1) on the same kernels")
+    ap.add_argument("--cycle", default="mfmg", choices=["mfmg", "v", "literal"],
+                    help="mfmg: the paper's HOMG cycle (default); v: classic V(2,1) on the same kernels; "
+                         "literal: the paper's own whole-grid design (one fine array, one launch per iteration)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the largest-3-D-grid roofline pass")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
@@ -120,10 +121,10 @@ def cycles_to_tol(hist_plus_final, cfg):
     return None, min(hist_plus_final) / n0
 
 
-def make_solver(cfg, inp, torch, dev, vcycle=None):
+def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False):
     from paper_1108_2045_b200 import homg
     s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters,
-                    schedule=cfg.schedule, device=dev, vcycle=vcycle)
+                    schedule=cfg.schedule, device=dev, vcycle=vcycle, literal=literal)
     tdt = torch.float64 if cfg.dtype == "f64" else torch.float32
     d = {k: (None if v is None else torch.from_numpy(v).to(dev)) for k, v in inp.items()}
     if d["k"] is not None:
@@ -273,7 +274,8 @@ def run_homg(args):
     if args.n:
         cfg = I.scaled(cfg, args.n)
     inp = I.make_inputs(cfg)
-    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None)
+    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None,
+                          literal=args.cycle == "literal")
     cstar, rel, stagnated, norms = find_cstar(s, d, cfg)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     sampler = ClockSampler(local)
@@ -359,7 +361,8 @@ def run_homg(args):
             "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": dict(workload_config(cfg), l2="flushed between steps (512 MiB write)",
-                           cycle="MFMG (HOMG)" if args.cycle == "mfmg" else "classic V(2,1)"),
+                           cycle={"mfmg": "MFMG (HOMG), per-level arrays", "v": "classic V(2,1)",
+                                  "literal": "MFMG (HOMG), paper-literal whole-grid iteration"}[args.cycle]),
             "cycles_to_tol": cstar, "rel_residual_reached": float(final[1]), "stagnated_above_tol": bool(stagnated),
             "ms_per_cycle": total_ms / args.steps / cstar,
             "unknowns_per_s_per_cycle": cfg.n_interior * world / (total_ms * 1e-3 / args.steps / cstar),
@@ -376,29 +379,32 @@ def run_homg(args):
         if not args.no_extra and world == 1 and not args.n and args.workload != "cfg4":
             line["roofline_largest_3d"] = extra_largest(torch, dev, peak, peak_src)
         if not args.no_extra and world == 1 and args.cycle == "mfmg":
-            line["classic_v21"] = extra_classic(torch, dev, cfg, inp, flush)
+            line["classic_v21"] = extra_other(torch, dev, cfg, inp, flush, vcycle=(2, 1))
+            line["paper_literal"] = extra_other(torch, dev, cfg, inp, flush, literal=True)
         print(json.dumps(line), flush=True)
     s.destroy()
     if world > 1:
         dist.destroy_process_group()
 
 
-def extra_classic(torch, dev, cfg, inp, flush):
-    """the comparison the paper argues: the same solve with the classic V(2,1)
-    cycle on the same hierarchy, operators and kernels (homg_options.cycle = HOMG_CYCLE_V)."""
-    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=(2, 1))
+def extra_other(torch, dev, cfg, inp, flush, vcycle=None, literal=False):
+    """the same solve with another cycle on the same hierarchy and operators: the classic V(2,1) cycle — the
+    comparison the paper argues — or the paper's own whole-grid design (Algorithm L:
+    one fine-grid array, one whole-grid launch per iteration, L51/L119), which the per-level layout replaces."""
+    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=vcycle, literal=literal)
     cstar, rel, stagnated, _ = find_cstar(s, d, cfg)
-    for _ in range(3):
+    reps = 2 if literal else 5
+    for _ in range(1 if literal else 3):
         s.set_initial_guess(d["u0"]); s.cycle(cstar); s.residual_norm()
     ms = 0.0
-    for _ in range(5):
+    for _ in range(reps):
         flush.zero_()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record()
         s.set_initial_guess(d["u0"]); s.cycle(cstar); fin = s.residual_norm()
         e1.record(); e1.synchronize()
         ms += e0.elapsed_time(e1)
-    ms /= 5
+    ms /= reps
     out = {"cycles_to_tol": cstar, "ms_per_step": ms, "ms_per_cycle": ms / cstar, "value": cfg.n_interior / (ms * 1e-3),
            "unit": UNIT, "rel_residual_reached": float(fin[1]), "stagnated_above_tol": bool(stagnated),
            "launches_per_cycle": s.launches_per_cycle()}

@@ -94,11 +94,15 @@ typedef struct {
     int cycle;        /* HOMG_CYCLE_MFMG (0, default): the paper's high-occupancy cycle;
                          HOMG_CYCLE_V (1): the classic V(v_eta1, v_eta2) cycle of PAPER.md L47 on the
                          same hierarchy, operators and kernels (exact solve on the coarsest level,
-                         which must then have exactly one interior node); schedule/max_iters unused */
+                         which must then have exactly one interior node); schedule/max_iters unused;
+                         HOMG_CYCLE_LITERAL (2): the paper's own design, same MFMG schedule and same
+                         numbers as HOMG_CYCLE_MFMG to rounding, but on ONE fine-grid array with one
+                         whole-fine-grid launch per iteration at every level — a
+                         measured prior-art row                                                        */
     int v_eta1;       /* pre-smoothing sweeps of HOMG_CYCLE_V; < 0: 2                    */
     int v_eta2;       /* post-smoothing sweeps of HOMG_CYCLE_V; < 0: 1                   */
 } homg_options;
-enum { HOMG_CYCLE_MFMG = 0, HOMG_CYCLE_V = 1 };
+enum { HOMG_CYCLE_MFMG = 0, HOMG_CYCLE_V = 1, HOMG_CYCLE_LITERAL = 2 };
 
 /* Fills *opt with the defaults (all "use default" markers). */
 HOMG_API void homg_default_options(homg_options* opt);

@@ -112,6 +112,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST_VAR")) s->fuse_first_var = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     s->vcycle = o.cycle == HOMG_CYCLE_V;
+    s->literal = o.cycle == HOMG_CYCLE_LITERAL;
     s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;
     s->v_eta2 = o.v_eta2 >= 0 ? o.v_eta2 : 1;
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);

@@ -13,6 +13,7 @@
 #include "homg_first.cuh"
 #include "homg_visit.cuh"
 #include "homg_moves.cuh"
+#include "homg_literal.cuh"
 
 namespace homg {
 
@@ -729,6 +730,42 @@ void rec_vcycle(Rec& R) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Paper-literal mode: Algorithm L on the GPU — one fine-grid array, one whole-grid
+// launch per iteration at every level.  A measured prior-art row, not the product.
+// ---------------------------------------------------------------------------------------------
+template <class T, int ND, bool VAR>
+void rec_literal(Rec& R) {
+    homg_solver* s = R.s;
+    const int M = s->levels - 1;
+    std::vector<Level>& L = s->L;
+    Level& L0 = L[0];
+    const bool have_g1 = rec_norm<T, ND, VAR>(R, true, true, true);           // r -> g_0, norm, g_1
+    for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
+        klaunch(R, k_restrict<T, ND>, grd(L[m].g), blk(), 0, L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);
+        R.check(TAG_RESTRICT);
+        R.acct(m - 1, 1.0, TAG_RESTRICT); R.acct(m, 1.0, TAG_RESTRICT);
+    }
+    int ic = 0, ip = 1, in = 2;                                                // cur, prev, nxt among the 3 level-0 buffers
+    cudaMemsetAsync(L0.rot[ic], 0, L0.n_alloc * sizeof(T), R.st); R.check(TAG_OTHER);
+    cudaMemsetAsync(L0.rot[ip], 0, L0.n_alloc * sizeof(T), R.st); R.check(TAG_OTHER);
+    R.acct(0, 2.0, TAG_OTHER);
+    for (size_t vi = 0; vi < s->sched_lv.size(); ++vi) {
+        const int m = s->sched_lv[vi];
+        for (int it = 0; it < s->sched_it[vi]; ++it) {
+            klaunch(R, k_iter_literal<T, ND, VAR>, grd(L0.g), blk(), 0, L0.g, L[m].g, m, make_coef<T>(s, m),
+                    (const T*)L0.rot[ic], (const T*)L0.rot[ip], (T*)L0.rot[in], (const T*)L[m].gsrc, faces<T>(L[m]));
+            R.check(m == 0 ? TAG_RELAX0 : TAG_RELAX);
+            R.acct(0, 3.0, m == 0 ? TAG_RELAX0 : TAG_RELAX);                   // 1 WU: read cur, prev; write nxt
+            const int t = ip; ip = ic; ic = in; in = t;
+        }
+    }
+    const long long n16 = (long long)(L0.n_alloc * sizeof(T) / 16);
+    klaunch(R, k_add_v<T>, dim3((unsigned)((n16 + 255) / 256)), dim3(256), 0, (T*)s->u, (const T*)L0.rot[ic], n16);
+    R.check(TAG_OTHER);
+    R.acct(0, 3.0, TAG_OTHER);
+}
+
 template <class T, int ND, bool VAR>
 void rec_sample(Rec& R) {
     homg_solver* s = R.s;
@@ -837,7 +874,7 @@ cudaError_t exec_init(homg_solver* s) {
 }
 
 cudaError_t exec_prepare(homg_solver* s) {
-    if (s->prog_ready || s->vcycle) return cudaSuccess;       // the V-cycle has no coarse program
+    if (s->prog_ready || s->vcycle || s->literal) return cudaSuccess;       // the V-cycle has no coarse program
     Rec P{s, s->stream};
     P.plan = true;
     HOMG_DISPATCH(s, rec_cycle, P);
@@ -855,6 +892,7 @@ cudaError_t exec_prepare(homg_solver* s) {
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     Rec R{s, st};
     if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
+    else if (s->literal) HOMG_DISPATCH(s, rec_literal, R);
     else HOMG_DISPATCH(s, rec_cycle, R);
     s->launches_per_cycle = R.launches;
     s->bytes_cycle_all = R.bytes_all;
@@ -873,6 +911,7 @@ cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_t
     Rec R{s, st};
     R.ev = &ev; R.ev_tag = &tag;
     if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
+    else if (s->literal) HOMG_DISPATCH(s, rec_literal, R);
     else HOMG_DISPATCH(s, rec_cycle, R);
     cudaError_t e = cudaStreamSynchronize(st);
     if (R.err == cudaSuccess) R.err = e;

@@ -75,6 +75,7 @@ struct homg_solver {
     bool fuse_first = true;          // fused interpolate+correct+relax first sweep (HOMG_FUSE_FIRST=0 disables)
     bool fuse_first_var = false;     // ... for the variable-coefficient stencil: measured slower than deliver + sweep
                                      // (cfg5: 535 us vs 64 + 190 us), off unless HOMG_FUSE_FIRST_VAR=1
+    bool literal = false;            // paper-literal whole-grid iteration, Algorithm L
     bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
     int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)

@@ -98,7 +98,7 @@ class Solver:
 
     def __init__(self, dims, levels, stencil, dtype, omega=0.0, h=0.0, max_iters=0, schedule=HOMG_SCHED_C,
                  sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, tiled_min_nodes=0,
-                 march_chunk=0, device="cuda:0", stream=None, vcycle=None):
+                 march_chunk=0, device="cuda:0", stream=None, vcycle=None, literal=False):
         import torch
         self._torch = torch
         self.dims = tuple(int(x) for x in dims)
@@ -116,6 +116,8 @@ class Solver:
         o.tiled_min_nodes, o.march_chunk = int(tiled_min_nodes), int(march_chunk)
         if vcycle is not None:                      # classic V(eta1, eta2) instead of the MFMG cycle
             o.cycle, o.v_eta1, o.v_eta2 = 1, int(vcycle[0]), int(vcycle[1])
+        if literal:                                 # the paper's whole-grid iteration (Algorithm L)
+            o.cycle = 2
         self._keep = None
         if sched is not None:
             lv, it = sched

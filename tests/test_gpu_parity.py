@@ -283,3 +283,33 @@ def test_vcycle_needs_one_node_coarsest_level():
     from paper_1108_2045_b200 import homg
     with pytest.raises(homg.HomgError):
         homg.Solver((65, 65, 65), 4, "poisson7", "f64", vcycle=(2, 1))
+
+
+# ---- paper-literal whole-grid mode (Algorithm L on the GPU) vs the oracle's Algorithm L ----
+@pytest.mark.parametrize("name,n,kind,maxi", [("cfg1", 65, 0, 4), ("cfg1", 33, 2, 2), ("cfg2", 17, 0, 4), ("cfg2", 33, 1, 8),
+                                              ("cfg4", 33, 0, 4), ("cfg5", 17, 0, 4), ("cfg3", 129, 0, 32)])
+def test_literal_mode(orc, name, n, kind, maxi):
+    import dataclasses
+    cfg = dataclasses.replace(I.scaled(I.CONFIGS[name], n), schedule=kind, max_iters=maxi)
+    inp = I.make_inputs(cfg)
+    ncyc = 3
+    us, norms, sched = run_gpu(cfg, inp, ncyc, literal=True)
+    osched = orc.schedule(cfg.schedule, cfg.levels, cfg.max_iters)
+    assert (list(sched[0]), list(sched[1])) == (list(osched[0]), list(osched[1]))
+    _, hist, onorms = orc.homg("L", inp["f"], inp["u0"], cfg.levels, cfg.omega, osched, ncyc, k=inp["k"])
+    tol = TOL[cfg.dtype]
+    for c in range(ncyc):
+        ref = hist[c].astype(np.float64)
+        err = np.max(np.abs(us[c].astype(np.float64) - ref)) / np.max(np.abs(ref))
+        assert err <= tol, f"{cfg.name} literal: cycle {c}: {err:.3e} > {tol}"
+    assert np.allclose(norms, onorms, rtol=1e-5 if cfg.dtype == "f32" else 1e-10)
+
+
+def test_literal_and_per_level_forms_agree(orc):
+    """Algorithm L (one fine array) and Algorithm H (per-level arrays, the product) give the same u to rounding (pin P7, on the GPU)."""
+    cfg = I.scaled(I.CONFIGS["cfg2"], 33)
+    inp = I.make_inputs(cfg)
+    a, _, _ = run_gpu(cfg, inp, 3, literal=True)
+    b, _, _ = run_gpu(cfg, inp, 3)
+    for x, y in zip(a, b):
+        assert np.max(np.abs(x - y)) <= 1e-12 * np.max(np.abs(y))
