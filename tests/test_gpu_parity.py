@@ -313,3 +313,21 @@ def test_literal_and_per_level_forms_agree(orc):
     b, _, _ = run_gpu(cfg, inp, 3)
     for x, y in zip(a, b):
         assert np.max(np.abs(x - y)) <= 1e-12 * np.max(np.abs(y))
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times (graph replay, default
+# ---- thresholds): the oracle runs the first cycle(s) of the same solve and EVERY node is compared ----
+@pytest.mark.parametrize("name,ncyc", [("cfg2", 4), ("cfg5", 3), ("cfg3", 2), ("cfg4", 2)])
+def test_full_size_first_cycles_vs_oracle(orc, name, ncyc):
+    cfg = I.CONFIGS[name]
+    inp = I.make_inputs(cfg)
+    us, norms, sched = run_gpu(cfg, inp, ncyc)
+    u_o, _, onorms = orc.homg("H", inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, ncyc, k=inp["k"], keep_history=False)
+    ref = u_o.astype(np.float64)
+    err = np.max(np.abs(us[-1].astype(np.float64) - ref)) / np.max(np.abs(ref))
+    assert err <= TOL[cfg.dtype], f"{name} full size: {err:.3e}"
+    assert np.allclose(norms, onorms, rtol=1e-5 if cfg.dtype == "f32" else 1e-10)
+    # Dirichlet boundary stays exactly 0
+    u = us[-1]
+    for ax in range(u.ndim):
+        assert not np.any(np.take(u, [0, -1], axis=ax))
