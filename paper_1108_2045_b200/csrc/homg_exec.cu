@@ -412,6 +412,10 @@ void rec_cycle(Rec& R) {
             }
             Lt.touched = true;
         } else {
+            // a deliver onto a large level whose hop also carries a step of the S3c prolongation (t >= 1) is
+            // held back and launched together with it (k_arrive_v): one launch per hop instead of two
+            struct PendingDeliver { bool on = false; const T* ec; const T* ac; T* ef; T* af; int ef_assign, af_mode; };
+            std::vector<PendingDeliver> pend(s->levels + 1);
             if (t < cur) {
                 // S3a deliver (interpolate + correct) level m -> m-1
                 for (int m = cur; m > t; --m) {
@@ -434,6 +438,8 @@ void rec_cycle(Rec& R) {
                         o.gi = Lc.g; o.p[0] = rotp<T>(Lc, Lc.e); o.p[1] = ac; o.q[0] = rotp<T>(Lf, Lf.e); o.q[1] = (T*)Lf.a;
                         o.f0 = ef_assign; o.f1 = af_mode;
                         R.push(o, Lf.n_nodes);
+                    } else if (t >= 1) {
+                        pend[m] = PendingDeliver{true, rotp<T>(Lc, Lc.e), ac, rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode};
                     } else {
                         flush();
                         if (!R.plan) klaunch(R, k_deliver_v<T, ND>, grdv<T>(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
@@ -493,6 +499,13 @@ void rec_cycle(Rec& R) {
                             o.gi = L[m].g; o.gv = Lv.g; o.s = last ? (1 << (cur - t)) : 0;
                             o.p[0] = A; o.p[1] = B; o.p[2] = X; o.p[3] = Y; o.q[0] = out;
                             R.push(o, L[m - 1].n_nodes);
+                        } else if (pend[m].on) {
+                            flush();
+                            const PendingDeliver& pd = pend[m];
+                            if (!R.plan) klaunch(R, k_arrive_v<T, ND>, grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, pd.ec, pd.ac, pd.ef,
+                                                 pd.af, pd.ef_assign, pd.af_mode, A, B, out, last ? (1 << (cur - t)) : 0,
+                                                 last ? cur - t : 0, Lv.g, X, Y);
+                            R.check(TAG_DELIVER);
                         } else {
                             flush();
                             if (!R.plan) klaunch(R, k_d0_down_v<T, ND>, grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,

@@ -58,13 +58,12 @@ __device__ __forceinline__ Pack<T> pack_interp(const LevelGeom& gc, const T* __r
     const int z = blockIdx.z;                                                   \
     if (x >= (g).nx || y >= (g).ny || z >= (g).nz) return;
 
-// k_deliver, one pack per thread.  grid = (ceil(nx / (32 VEC)), ceil(ny / 8), nz), block (32, 8).
+// k_deliver for the pack x..x+VEC-1 of row (y, z)
 template <class T, int ND>
-__global__ void __launch_bounds__(256)
-k_deliver_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, const T* __restrict__ ac, T* __restrict__ ef,
-            T* __restrict__ af, int ef_assign, int af_mode) {
-    pdl_start();
-    HOMG_PACK_XYZ(gf);
+__device__ __forceinline__ void deliver_pack(const LevelGeom& gf, const LevelGeom& gc, const T* __restrict__ ec,
+                                             const T* __restrict__ ac, T* __restrict__ ef, T* __restrict__ af,
+                                             int ef_assign, int af_mode, int x, int y, int z) {
+    constexpr int VEC = 16 / int(sizeof(T));
     const long long c = lidx(gf, x, y, z);
     Pack<T> inc;
     if (ac) inc = pack_interp<T, ND>(gc, ac, nullptr, x, y, z);
@@ -93,13 +92,13 @@ k_deliver_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, const T* __res
     }
 }
 
-// k_d0_down, one pack per thread; coin_s is 0 or a power of two (sh = log2 coin_s).
+// k_d0_down for one pack; coin_s is 0 or a power of two (sh = log2 coin_s)
 template <class T, int ND>
-__global__ void __launch_bounds__(256)
-k_d0_down_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, const T* __restrict__ B, T* __restrict__ out,
-            int coin_s, int sh, LevelGeom gv, const T* __restrict__ X, const T* __restrict__ Y) {
-    pdl_start();
-    HOMG_PACK_XYZ(gf);
+__device__ __forceinline__ void d0_down_pack(const LevelGeom& gf, const LevelGeom& gc, const T* __restrict__ A,
+                                             const T* __restrict__ B, T* __restrict__ out, int coin_s, int sh,
+                                             const LevelGeom& gv, const T* __restrict__ X, const T* __restrict__ Y,
+                                             int x, int y, int z) {
+    constexpr int VEC = 16 / int(sizeof(T));
     Pack<T> val = pack_interp<T, ND>(gc, A, B, x, y, z);
     const int mask = coin_s - 1;
     const bool rowcoin = coin_s > 0 && !(y & mask) && (ND == 2 || !(z & mask));
@@ -112,6 +111,38 @@ k_d0_down_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, const T* __rest
         }
     }
     *reinterpret_cast<Pack<T>*>(out + lidx(gf, x, y, z)) = val;
+}
+
+// one pack per thread.  grid = (ceil(nx / (32 VEC)), ceil(ny / 8), nz), block (32, 8).
+template <class T, int ND>
+__global__ void __launch_bounds__(256)
+k_deliver_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, const T* __restrict__ ac, T* __restrict__ ef,
+            T* __restrict__ af, int ef_assign, int af_mode) {
+    pdl_start();
+    HOMG_PACK_XYZ(gf);
+    deliver_pack<T, ND>(gf, gc, ec, ac, ef, af, ef_assign, af_mode, x, y, z);
+}
+
+template <class T, int ND>
+__global__ void __launch_bounds__(256)
+k_d0_down_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ A, const T* __restrict__ B, T* __restrict__ out,
+            int coin_s, int sh, LevelGeom gv, const T* __restrict__ X, const T* __restrict__ Y) {
+    pdl_start();
+    HOMG_PACK_XYZ(gf);
+    d0_down_pack<T, ND>(gf, gc, A, B, out, coin_s, sh, gv, X, Y, x, y, z);
+}
+
+// one hop level m -> m-1 on the way down to a visit: S3a deliver and the S3c prolongation step of the
+// carried variation have the same grid and independent outputs — one launch instead of two
+template <class T, int ND>
+__global__ void __launch_bounds__(256)
+k_arrive_v(LevelGeom gf, LevelGeom gc, const T* __restrict__ ec, const T* __restrict__ ac, T* __restrict__ ef,
+           T* __restrict__ af, int ef_assign, int af_mode, const T* __restrict__ A, const T* __restrict__ B,
+           T* __restrict__ out, int coin_s, int sh, LevelGeom gv, const T* __restrict__ X, const T* __restrict__ Y) {
+    pdl_start();
+    HOMG_PACK_XYZ(gf);
+    deliver_pack<T, ND>(gf, gc, ec, ac, ef, af, ef_assign, af_mode, x, y, z);
+    d0_down_pack<T, ND>(gf, gc, A, B, out, coin_s, sh, gv, X, Y, x, y, z);
 }
 
 // Classic V-cycle, step (d): v += S^ e_c on every node (coincident nodes add e_c itself,
