@@ -414,6 +414,9 @@ void rec_cycle(Rec& R) {
         } else {
             // a deliver onto a large level whose hop also carries a step of the S3c prolongation (t >= 1) is
             // held back and launched together with it (k_arrive_v): one launch per hop instead of two
+            bool inj_pending = false;                               // the last inject of a move up (level t-1 -> t, t large)
+            const T* inj_src = nullptr;
+            T* inj_dst = nullptr;
             struct PendingDeliver { bool on = false; const T* ec; const T* ac; T* ef; T* af; int ef_assign, af_mode; };
             std::vector<PendingDeliver> pend(s->levels + 1);
             if (t < cur) {
@@ -460,6 +463,9 @@ void rec_cycle(Rec& R) {
                         CoarseOp<T> o = newop(OP_INJECT, m);
                         o.gi = L[m - 1].g; o.p[0] = rotp<T>(L[m - 1], L[m - 1].e); o.q[0] = rotp<T>(L[m], L[m].e);
                         R.push(o, L[m].n_nodes);
+                    } else if (m == t) {
+                        inj_pending = true;                         // launched together with k_d0_up below (k_rise)
+                        inj_src = rotp<T>(L[m - 1], L[m - 1].e); inj_dst = rotp<T>(L[m], L[m].e);
                     } else {
                         flush();
                         if (!R.plan) klaunch(R, k_inject<T, ND>, grd(L[m].g), blk(), 0, L[m].g, L[m - 1].g, rotp<T>(L[m - 1], L[m - 1].e),
@@ -481,6 +487,12 @@ void rec_cycle(Rec& R) {
                         CoarseOp<T> o = newop(OP_D0_UP, t);
                         o.gi = Lv.g; o.s = 1 << (t - cur); o.p[0] = X; o.p[1] = Y; o.q[0] = (T*)Lt.d0;
                         R.push(o, Lt.n_nodes);
+                    } else if (inj_pending) {
+                        flush();
+                        if (!R.plan) klaunch(R, k_rise<T, ND>, grd(Lt.g), blk(), 0, Lt.g, L[t - 1].g, inj_src, inj_dst, Lv.g, 1 << (t - cur),
+                                             X, Y, (T*)Lt.d0);
+                        R.check(TAG_INJECT);
+                        inj_pending = false;
                     } else {
                         flush();
                         if (!R.plan) klaunch(R, k_d0_up<T, ND>, grd(Lt.g), blk(), 0, Lt.g, Lv.g, 1 << (t - cur), X, Y, (T*)Lt.d0);

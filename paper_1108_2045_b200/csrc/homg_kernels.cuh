@@ -262,6 +262,19 @@ __global__ void k_d0_up(LevelGeom gt, LevelGeom gv, int s, const T* __restrict__
     d0[lidx(gt, x, y, z)] = X[q] - Y[q];
 }
 
+// a move up that ends on level t: the last inject (level t-1 -> t) and k_d0_up have the same grid and
+// independent outputs — one launch instead of two
+template <class T, int ND>
+__global__ void k_rise(LevelGeom gt, LevelGeom gf, const T* __restrict__ ef, T* __restrict__ ec, LevelGeom gv, int s,
+                       const T* __restrict__ X, const T* __restrict__ Y, T* __restrict__ d0) {
+    pdl_start();
+    HOMG_NODE_XYZ(gt);
+    const long long c = lidx(gt, x, y, z);
+    ec[c] = ef[lidx(gf, 2 * x, 2 * y, ND == 3 ? 2 * z : 0)];
+    const long long q = lidx(gv, x * s, y * s, ND == 3 ? z * s : 0);
+    d0[c] = X[q] - Y[q];
+}
+
 // one prolongation step of the carried variation going finer: out = S^(A - B) on the fine level;
 // on the last step (coin_s > 0) nodes coincident with level v (all indices multiples of coin_s)
 // take dl = X - Y of level v instead.  Grid over the FINE level.               (S3c)
