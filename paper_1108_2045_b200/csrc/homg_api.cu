@@ -102,6 +102,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
                                                        : (o.coarse_threshold_nodes < 0 ? 0 : kCoarseNodesDefault);
     if (const char* ev = std::getenv("HOMG_COARSE_NODES")) s->coarse_threshold = std::atoll(ev);
     if (const char* ev = std::getenv("HOMG_COARSE_CLUSTER")) s->coarse_cluster = std::atoi(ev);
+    if (const char* ev = std::getenv("HOMG_COARSE_RELAXN")) s->coarse_relaxn = std::atoi(ev) != 0;
     s->use_graph = o.use_graph != 0;
     s->tiled_min_nodes = o.tiled_min_nodes > 0 ? o.tiled_min_nodes : (o.tiled_min_nodes < 0 ? -1 : kTiledMinNodesDefault);
     if (const char* ev = std::getenv("HOMG_TILED_MIN_NODES")) s->tiled_min_nodes = std::atoll(ev);

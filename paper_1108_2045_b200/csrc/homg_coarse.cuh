@@ -17,7 +17,9 @@
 
 namespace homg {
 
-enum { OP_ZERO = 0, OP_RESTRICT, OP_DELIVER, OP_INJECT, OP_D0_UP, OP_D0_DOWN, OP_RELAX };
+enum { OP_ZERO = 0, OP_RESTRICT, OP_DELIVER, OP_INJECT, OP_D0_UP, OP_D0_DOWN, OP_RELAX, OP_RELAXN };
+
+constexpr int kRelaxnSmemMax = 176 * 1024;   // dynamic shared memory an OP_RELAXN may ask for
 
 template <class T>
 struct CoarseOp {
@@ -30,6 +32,7 @@ struct CoarseOp {
     Faces<T> kf;              // OP_RELAX, variable coefficient
     const T* p[5];
     T* q[3];
+    T* qx[2];                 // OP_RELAXN: where v^{eta-1} and v^{eta-2} go (q[0]: v^eta); null = not kept
 };
 
 constexpr int kMaxRunOps = 96;   // records staged in shared memory per launch; longer runs are split
@@ -185,6 +188,83 @@ __device__ __forceinline__ void coarse_node(const CoarseOp<T>& o, int x, int y, 
 
 #undef ldcg
 
+// OP_RELAXN: ALL `o.s` = eta sweeps of a visit on a small level by one CTA, the iterate kept in shared
+// memory between sweeps (compact nx*ny*nz layout: two ping-pong copies of v and one of g), one CTA
+// barrier per sweep instead of one record (and one L2 round trip) per sweep.  Only the last three
+// iterates are written to their global buffers (the next visit's carried variation reads them, S3c);
+// the last sweep carries the epilogues of OP_RELAX.  Same arithmetic, node by node, as OP_RELAX.
+template <class T, int ND, bool VAR, bool CG>
+__device__ void coarse_relaxn(const CoarseOp<T>& o, T* sm) {
+    const LevelGeom& g = o.go;
+    const int nx = g.nx, ny = g.ny, nz = g.nz, N = nx * ny * nz, eta = o.s;
+    const int sy = nx, sz = nx * ny;
+    T* bufA = sm;
+    T* bufB = sm + N;
+    T* gs = sm + 2 * N;
+    for (int n = threadIdx.x; n < N; n += blockDim.x) {
+        const int x = n % nx, t = n / nx;
+        const long long c = lidx(g, x, t % ny, t / ny);
+        bufA[n] = ldg_<CG>(o.p[0] + c);
+        gs[n] = ldg_<CG>(o.p[1] + c);
+    }
+    __syncthreads();
+    long long c = 0;
+    bool inner = false;
+    for (int it = 0; it < eta; ++it) {
+        const T* vin = (it & 1) ? bufB : bufA;
+        T* vout = (it & 1) ? bufA : bufB;
+        const bool last = it == eta - 1;
+        T* gout = last ? o.q[0] : (it == eta - 2 ? o.qx[0] : (it == eta - 3 ? o.qx[1] : nullptr));
+        T* a = last ? o.q[1] : nullptr;
+        T* u = last ? o.q[2] : nullptr;
+        for (int n = threadIdx.x; n < N; n += blockDim.x) {
+            // (the integer divisions are a long dependent chain: a thread with a single node keeps its
+            // coordinates from the first sweep)
+            if (it == 0 || N > int(blockDim.x)) {
+                const int x = n % nx, t = n / nx, y = t % ny, z = t / ny;
+                c = lidx(g, x, y, z);
+                inner = is_interior<ND>(g, x, y, z);
+            }
+            if (!inner) {
+                vout[n] = T(0);
+                if (gout) gout[c] = T(0);
+                if (a && o.f0) a[c] = T(0);
+                continue;
+            }
+            const T vc = vin[n];
+            T vn;
+            if (!VAR) {
+                T s = T(0);
+                if (ND == 3) s += vin[n - sz] + vin[n + sz];
+                s += vin[n - sy] + vin[n + sy];
+                s += vin[n - 1] + vin[n + 1];
+                vn = jacobi_eq3(vc, s, gs[n], o.cf);
+            } else {
+                T acc = T(0), dsum = T(0);
+                const int st[3] = {sz, sy, 1};
+                const long long off[3] = {g.pp, (long long)g.px, 1};
+                const T* fa[3] = {o.kf.z, o.kf.y, o.kf.x};
+#pragma unroll
+                for (int ax = 3 - ND; ax < 3; ++ax) {
+                    const T fm = fa[ax][c - off[ax]], fp = fa[ax][c];
+                    acc += fm * (vc - vin[n - st[ax]]); dsum += fm;
+                    acc += fp * (vc - vin[n + st[ax]]); dsum += fp;
+                }
+                const T Av = acc * o.cf.ih2, D = dsum * o.cf.ih2;
+                vn = vc + o.cf.w * (gs[n] - Av) / D;
+            }
+            vout[n] = vn;
+            if (gout) gout[c] = vn;
+            if (a) {
+                const T Dq = ((o.p[3] ? ldg_<CG>(o.p[3] + c) : T(0)) + vc) - ldg_<CG>(o.p[4] + c);
+                a[c] = o.f0 ? Dq : ldg_<CG>(a + c) + Dq;
+            }
+            if (u) u[c] = ldg_<CG>(u + c) + vn;
+        }
+        __syncthreads();
+    }
+}
+
 // One launch = one cluster of gridDim.x CTAs x 1024 threads running ops[0..nops), nops <= kMaxRunOps.
 // MULTI = (gridDim.x > 1).  Operations on tiny levels (act = 1) are worked by CTA 0 alone and
 // separated by a CTA barrier; everything else by the whole cluster and a cluster barrier.
@@ -194,6 +274,7 @@ __global__ void __launch_bounds__(1024) k_coarse_run(const CoarseOp<T>* __restri
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     __shared__ CoarseOp<T> sops[kMaxRunOps];
+    extern __shared__ uint4 relaxn_smem[];                // OP_RELAXN: 3 compact copies of a small level
     {   // the records were written by the host before the launch: plain loads are safe
         const int words = nops * int(sizeof(CoarseOp<T>) / 4);
         for (int w = threadIdx.x; w < words; w += blockDim.x)
@@ -208,6 +289,8 @@ __global__ void __launch_bounds__(1024) k_coarse_run(const CoarseOp<T>* __restri
             const unsigned gt = solo ? threadIdx.x : blockIdx.x * blockDim.x + threadIdx.x;
             if (op.type == OP_ZERO) {
                 for (long long n = gt; n < op.count; n += nth) op.q[0][n] = T(0);
+            } else if (op.type == OP_RELAXN) {             // act = 1: this CTA alone
+                coarse_relaxn<T, ND, VAR, MULTI>(op, reinterpret_cast<T*>(relaxn_smem));
             } else {
                 const int nx = op.go.nx, ny = op.go.ny;
                 const int total = nx * ny * op.go.nz;

@@ -292,7 +292,15 @@ void flush_run(Rec& R) {
         for (int b = 0; b < R.run_len; b += kMaxRunOps) {       // long runs: kMaxRunOps records per launch
             const int n = std::min(kMaxRunOps, R.run_len - b);
             const CoarseOp<T>* dev = static_cast<const CoarseOp<T>*>(s->prog_dev) + R.run_begin + b;
+            size_t smem = 0;                                     // OP_RELAXN: 3 compact copies of its level
+            {
+                const CoarseOp<T>* hops = reinterpret_cast<const CoarseOp<T>*>(R.prog.data()) + R.run_begin + b;
+                for (int i = 0; i < n; ++i)
+                    if (hops[i].type == OP_RELAXN)
+                        smem = std::max(smem, 3 * size_t(hops[i].go.nx) * hops[i].go.ny * hops[i].go.nz * sizeof(T));
+            }
             cudaLaunchConfig_t cfg = {};
+            cfg.dynamicSmemBytes = smem;
             cfg.gridDim = dim3(ncta, 1, 1);
             cfg.blockDim = dim3(1024, 1, 1);
             cfg.stream = R.st;
@@ -607,6 +615,38 @@ void rec_cycle(Rec& R) {
         // into the last sweep of the cycle.
         const int v0 = Lt.e;
         int in = v0, prev_in = -1, prev2 = -1;
+        // a small level whose compact arrays fit in one CTA's shared memory: the whole visit is ONE record
+        // of the coarse program (OP_RELAXN), the iterate stays in shared memory between the sweeps
+        if (small(t) && eta >= 2 && s->coarse_relaxn &&
+            3 * size_t(Lt.n_nodes) * sizeof(T) <= size_t(kRelaxnSmemMax)) {
+            std::vector<int> outs(eta);
+            for (int it = 0; it < eta; ++it) {
+                int out = -1;
+                for (int b = 0; b < Lt.nrot; ++b)
+                    if (b != in && b != prev_in && !(t >= 1 && b == v0)) { out = b; break; }
+                outs[it] = out;
+                prev2 = prev_in; prev_in = in; in = out;
+            }
+            const bool book = t >= 1, addu = vi == nv - 1;
+            CoarseOp<T> o = newop(OP_RELAXN, t);
+            o.cf = make_coef<T>(s, t);
+            o.s = eta;
+            o.p[0] = rotp<T>(Lt, v0); o.p[1] = (const T*)Lt.gsrc; o.p[2] = nullptr; o.kf = faces<T>(Lt);
+            o.p[3] = have_d0 ? (const T*)Lt.d0 : nullptr; o.p[4] = rotp<T>(Lt, v0);
+            o.q[0] = rotp<T>(Lt, outs[eta - 1]); o.q[1] = book ? (T*)Lt.a : nullptr; o.q[2] = addu ? (T*)s->u : nullptr;
+            o.qx[0] = rotp<T>(Lt, outs[eta - 2]);
+            o.qx[1] = eta >= 3 ? rotp<T>(Lt, outs[eta - 3]) : nullptr;
+            o.f0 = a_zero[t] ? 1 : 0;
+            R.push(o, 1);                                    // act = 1: worked by one CTA
+            if (Lt.n_nodes > R.run_maxnodes) R.run_maxnodes = Lt.n_nodes;
+            R.acct(t, 3.0 * eta + (VAR ? 3.0 * eta : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + 1.0 : 0.0) +
+                          (addu ? 2.0 : 0.0), TAG_COARSE);
+            if (t >= 1) a_zero[t] = 0;
+            Lt.vk = in; Lt.vkm1 = prev_in; Lt.vkm2 = prev2; Lt.e = in; Lt.eta_last = eta;
+            dp_is_d0[t] = false;
+            cur = t;
+            continue;
+        }
         for (int it = 0; it < eta; ++it) {
             int out = -1;
             for (int b = 0; b < Lt.nrot; ++b)
@@ -856,6 +896,13 @@ cudaError_t set_attr() {
                                 res_smem_bytes<T, ND, VAR>());
 }
 
+template <class T, int ND, bool VAR>
+cudaError_t set_attr_coarse() {
+    cudaError_t e = cudaFuncSetAttribute(k_coarse_run<T, ND, VAR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRelaxnSmemMax);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_coarse_run<T, ND, VAR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRelaxnSmemMax);
+}
+
 template <class T, int ND, int NS>
 cudaError_t set_attr_visit1() {
     cudaError_t e = cudaFuncSetAttribute(k_visit<T, ND, NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -889,6 +936,12 @@ cudaError_t exec_init(homg_solver* s) {
     if ((e = set_attr<double, 2, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, true>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<float, 2, false>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<float, 3, false>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<float, 3, true>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<double, 2, false>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<double, 3, false>()) != cudaSuccess) return e;
+    if ((e = set_attr_coarse<double, 3, true>()) != cudaSuccess) return e;
     if ((e = set_attr_visit<float, 2>()) != cudaSuccess) return e;
     if ((e = set_attr_visit<float, 3>()) != cudaSuccess) return e;
     if ((e = set_attr_visit<float, 4>()) != cudaSuccess) return e;

@@ -68,6 +68,7 @@ struct homg_solver {
     int coarse_cluster = 0;          // 0: automatic cluster size (1, 4 or 8 CTAs)
     void* prog_dev = nullptr;        // CoarseOp records of one cycle (library-owned device memory)
     bool prog_ready = false;
+    bool coarse_relaxn = true;       // a visit of a small level = one OP_RELAXN record (HOMG_COARSE_RELAXN=0: one record per sweep)
     bool use_graph = true;
     long long tiled_min_nodes = 0;   // levels with >= this many nodes use the TMA-tiled kernels
     int march_chunk = 0;             // 0: automatic
