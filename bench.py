@@ -43,6 +43,10 @@ def parse():
     ap.add_argument("--cycle", default="mfmg", choices=["mfmg", "v", "literal"],
                     help="mfmg: the paper's HOMG cycle (default); v: classic V(2,1) on the same kernels; "
                          "literal: the paper's own whole-grid design (one fine array, one launch per iteration)")
+    ap.add_argument("--mixed", action="store_true",
+                    help="mixed-precision outer loop (SURVEY.md 8(f)2): u, f, residual in fp64, the correction cycle in "
+                         "fp32; the workload's inputs are generated in fp64 (cfg3/cfg4: makes tolerances below the "
+                         "fp32 floor reachable; cfg2/cfg5: halves the sweep traffic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the largest-3-D-grid roofline pass")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
@@ -121,10 +125,10 @@ def cycles_to_tol(hist_plus_final, cfg):
     return None, min(hist_plus_final) / n0
 
 
-def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False):
+def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False, mixed=False):
     from paper_1108_2045_b200 import homg
     s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters,
-                    schedule=cfg.schedule, device=dev, vcycle=vcycle, literal=literal)
+                    schedule=cfg.schedule, device=dev, vcycle=vcycle, literal=literal, mixed=mixed)
     tdt = torch.float64 if cfg.dtype == "f64" else torch.float32
     d = {k: (None if v is None else torch.from_numpy(v).to(dev)) for k, v in inp.items()}
     if d["k"] is not None:
@@ -273,9 +277,12 @@ def run_homg(args):
     cfg = I.CONFIGS[args.workload]
     if args.n:
         cfg = I.scaled(cfg, args.n)
+    if args.mixed:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, dtype="f64")
     inp = I.make_inputs(cfg)
     s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None,
-                          literal=args.cycle == "literal")
+                          literal=args.cycle == "literal", mixed=args.mixed)
     cstar, rel, stagnated, norms = find_cstar(s, d, cfg)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     sampler = ClockSampler(local)
@@ -341,12 +348,14 @@ def run_homg(args):
     sampler.mark(t_b, time.time())
 
     # ---- per-kernel timing (CUDA events after every launch, plain stream launches) ----
-    s.set_initial_guess(d["u0"])
-    s.profile_cycles(1)                         # warm
-    s.set_initial_guess(d["u0"])
-    t_c = time.time()
-    prof = s.profile_cycles(cstar)
-    sampler.mark(t_c, time.time())
+    prof = {}
+    if not args.mixed:                          # (homg_profile_cycles is not available in mixed precision)
+        s.set_initial_guess(d["u0"])
+        s.profile_cycles(1)                     # warm
+        s.set_initial_guess(d["u0"])
+        t_c = time.time()
+        prof = s.profile_cycles(cstar)
+        sampler.mark(t_c, time.time())
     peak, peak_src = peaks()
     comp, comp_total = s.compulsory_bytes_per_cycle()
     rl, shares = roofline_from_profile(prof, peak, peak_src, comp, cstar, cfg.name)
@@ -359,7 +368,8 @@ def run_homg(args):
     nbytes = int(np.prod(cfg.dims)) * es
     line = {"metric": METRIC, "value": replicas.job_value(cfg.n_interior, args.steps, world, total_ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64 (u, f, residual) / f32 (correction cycle)" if args.mixed else cfg.dtype, "data": "synthetic",
             "config": dict(workload_config(cfg), l2="flushed between steps (512 MiB write)",
                            cycle={"mfmg": "MFMG (HOMG), per-level arrays", "v": "classic V(2,1)",
                                   "literal": "MFMG (HOMG), paper-literal whole-grid iteration"}[args.cycle]),
@@ -376,9 +386,9 @@ def run_homg(args):
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(cfg, inp, cstar, args.cpu_seconds)
-        if not args.no_extra and world == 1 and not args.n and args.workload != "cfg4":
+        if not args.no_extra and world == 1 and not args.n and args.workload != "cfg4" and not args.mixed:
             line["roofline_largest_3d"] = extra_largest(torch, dev, peak, peak_src)
-        if not args.no_extra and world == 1 and args.cycle == "mfmg":
+        if not args.no_extra and world == 1 and args.cycle == "mfmg" and not args.mixed:
             line["classic_v21"] = extra_other(torch, dev, cfg, inp, flush, vcycle=(2, 1))
             line["paper_literal"] = extra_other(torch, dev, cfg, inp, flush, literal=True)
         print(json.dumps(line), flush=True)

@@ -101,11 +101,20 @@ typedef struct {
                          measured prior-art row                                                        */
     int v_eta1;       /* pre-smoothing sweeps of HOMG_CYCLE_V; < 0: 2                    */
     int v_eta2;       /* post-smoothing sweeps of HOMG_CYCLE_V; < 0: 1                   */
+    int mixed;        /* 1: mixed-precision outer loop (the restart of the cycles is a
+                         defect-correction loop).  dtype must be HOMG_F64: u, f, k,
+                         the residual r = f - A u and u += e are fp64; r is rounded to fp32 and ONE fp32
+                         HOMG cycle on A e = r from e = 0 gives the correction.  The workspace must
+                         hold homg_workspace_bytes_mixed() bytes.                                   */
 } homg_options;
 enum { HOMG_CYCLE_MFMG = 0, HOMG_CYCLE_V = 1, HOMG_CYCLE_LITERAL = 2 };
 
 /* Fills *opt with the defaults (all "use default" markers). */
 HOMG_API void homg_default_options(homg_options* opt);
+
+/* Bytes of device workspace a mixed-precision solver (homg_options.mixed = 1) needs: the fp64 level-0
+ * arrays plus the fp32 hierarchy (0 on bad arguments). */
+HOMG_API size_t homg_workspace_bytes_mixed(int ndim, const int64_t* dims, int levels, homg_stencil stencil);
 
 /* Bytes of device workspace homg_create needs for this hierarchy (0 on bad arguments).
  * Layout: DESIGN.md "Data layout in HBM" — every level array is contiguous, rows padded

@@ -661,6 +661,37 @@ int run_vcycle(int nd, const int64_t* dims, int levels, double h, const void* kc
     return 0;
 }
 
+// ---------------------------------------------------------------------------
+// Mixed-precision outer loop.  PAPER.md L75: "the residual equation is used to restart
+// the cycles" — the restart is a defect-correction loop, so the correction cycle may run in a lower
+// precision than the residual:  u, f and r = f - A u in fp64;  r rounded to fp32;  ONE HOMG cycle in fp32
+// on A e = r from e = 0 (Algorithm H, coefficient k rounded to fp32);  u += e in fp64.
+// ---------------------------------------------------------------------------
+int run_homg_mixed(int nd, const int64_t* dims, int levels, double h, const double* kc, double omega,
+                   const int* slv, const int* sit, int slen, const double* f, double* u, int ncycles,
+                   double* u_hist, double* norms) {
+    Hier<double> Hd;
+    if (!build_hier<double>(Hd, nd, dims, levels, h, kc)) return 1;
+    const Grid& F = Hd.G[0];
+    const int64_t N = F.size();
+    std::vector<float> k32;
+    if (kc) { k32.resize(N); for (int64_t i = 0; i < N; ++i) k32[i] = float(kc[i]); }
+    Hier<float> Hf;
+    if (!build_hier<float>(Hf, nd, dims, levels, h, kc ? k32.data() : nullptr)) return 1;
+    std::vector<double> r(N);
+    std::vector<float> r32(N), e32(N);
+    for (int c = 0; c < ncycles; ++c) {
+        double n2 = residual(F, h, Hd.kptr(0), u, f, r.data());
+        if (norms) norms[c] = std::sqrt(n2);
+        for (int64_t i = 0; i < N; ++i) { r32[i] = float(r[i]); e32[i] = 0.0f; }
+        cycle_H<float>(Hf, omega, slv, sit, slen, r32.data(), e32.data());
+        for (int64_t i = 0; i < N; ++i) u[i] += double(e32[i]);
+        if (u_hist) std::memcpy(u_hist + int64_t(c) * N, u, sizeof(double) * N);
+    }
+    if (norms) norms[ncycles] = std::sqrt(residual(F, h, Hd.kptr(0), u, f, (double*)nullptr));
+    return 0;
+}
+
 }  // namespace
 
 #define DISPATCH(dtype, CALL32, CALL64) ((dtype) == 4 ? (CALL32) : (dtype) == 8 ? (CALL64) : -1)
@@ -730,6 +761,12 @@ int orc_homg(int alg, int dtype, int nd, const int64_t* dims, int levels, double
     if (dtype == 4) return run_homg<float>(alg, nd, dims, levels, h, k, omega, slv, sit, slen, f, u, ncycles, u_hist, norms);
     if (dtype == 8) return run_homg<double>(alg, nd, dims, levels, h, k, omega, slv, sit, slen, f, u, ncycles, u_hist, norms);
     return -1;
+}
+
+// mixed-precision outer loop: fp64 u, f, k; the correction cycle in fp32 (Algorithm H)
+int orc_homg_mixed(int nd, const int64_t* dims, int levels, double h, const double* k, double omega, const int* slv,
+                   const int* sit, int slen, const double* f, double* u, int ncycles, double* u_hist, double* norms) {
+    return run_homg_mixed(nd, dims, levels, h, k, omega, slv, sit, slen, f, u, ncycles, u_hist, norms);
 }
 
 // the first `niters` whole-grid iterations of ONE literal cycle started from u;

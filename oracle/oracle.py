@@ -118,6 +118,20 @@ def homg(alg, f, u0, levels, omega, sched, ncycles, h=None, k=None, keep_history
     return u, hist, norms
 
 
+def homg_mixed(f, u0, levels, omega, sched, ncycles, h=None, k=None, keep_history=True):
+    """mixed-precision outer loop: fp64 u, f, residual; one fp32 HOMG cycle (Algorithm H) per
+    outer cycle on the residual equation.  Returns (u, u_hist or None, norms[ncycles+1])."""
+    f = _c(f, np.float64); u = np.array(u0, dtype=np.float64, order="C", copy=True); k = _c(k, np.float64)
+    hist = np.empty((ncycles,) + f.shape, dtype=np.float64) if keep_history else None
+    norms = np.zeros(ncycles + 1, dtype=np.float64)
+    lv, it, n = _sched_arrays(sched)
+    rc = lib().orc_homg_mixed(f.ndim, _dims(f.shape), levels, C.c_double(h or default_h(f.shape)), _p(k),
+                              C.c_double(omega), lv, it, n, _p(f), _p(u), ncycles, _p(hist),
+                              norms.ctypes.data_as(C.POINTER(C.c_double)))
+    assert rc == 0, rc
+    return u, hist, norms
+
+
 def homg_L_partial(f, u0, levels, omega, sched, niters, h=None, k=None):
     """correction array after the first `niters` whole-grid iterations of one literal cycle (fp64)."""
     f = _c(f, np.float64); u = _c(u0, np.float64); k = _c(k, np.float64)

@@ -76,9 +76,44 @@ size_t homg_workspace_bytes(int ndim, const int64_t* dims, int levels, homg_sten
     return P.total_bytes + round_up(size_t(4096) * sizeof(double), 256);   // default history
 }
 
+static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, int levels, homg_stencil st,
+                              homg_dtype dt, void* ws, size_t ws_bytes, const homg_options* opt);
+
+size_t homg_workspace_bytes_mixed(int ndim, const int64_t* dims, int levels, homg_stencil st) {
+    const size_t a = homg_workspace_bytes(ndim, dims, 1, st, HOMG_F64);
+    const size_t b = homg_workspace_bytes(ndim, dims, levels, st, HOMG_F32);
+    return (a && b) ? round_up(a, 256) + b : 0;
+}
+
 homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int levels, homg_stencil st,
                         homg_dtype dt, void* ws, size_t ws_bytes, const homg_options* opt) {
     if (!out) return set_err(nullptr, HOMG_EINVAL, "out is null");
+    *out = nullptr;
+    if (!opt || !opt->mixed) return create_one(out, ndim, dims, levels, st, dt, ws, ws_bytes, opt);
+    // mixed precision: an fp64 one-level outer problem (u, f, r) + the fp32 hierarchy of the correction cycle
+    if (dt != HOMG_F64) return set_err(nullptr, HOMG_EINVAL, "mixed precision: dtype must be HOMG_F64 (u, f, k are fp64)");
+    if (opt->cycle != HOMG_CYCLE_MFMG) return set_err(nullptr, HOMG_EINVAL, "mixed precision runs the MFMG cycle only");
+    homg_options o = *opt;
+    o.mixed = 0;
+    const size_t extra = o.history_cap > 4096 ? round_up(size_t(o.history_cap - 4096) * sizeof(double), 256) : 0;
+    const size_t a = homg_workspace_bytes(ndim, dims, 1, st, HOMG_F64), b = homg_workspace_bytes(ndim, dims, levels, st, HOMG_F32);
+    if (!a || !b) return set_err(nullptr, HOMG_EINVAL, g_create_err);
+    const size_t a_al = round_up(a + extra, 256);
+    if (!ws) return set_err(nullptr, HOMG_EINVAL, "workspace is null");
+    if (ws_bytes < a_al + b + extra) return set_err(nullptr, HOMG_ENOMEM, "workspace too small (see homg_workspace_bytes_mixed)");
+    homg_solver* outer = nullptr;
+    homg_solver* inner = nullptr;
+    homg_status r = create_one(&outer, ndim, dims, 1, st, HOMG_F64, ws, a_al, &o);
+    if (r != HOMG_OK) return r;
+    r = create_one(&inner, ndim, dims, levels, st, HOMG_F32, static_cast<char*>(ws) + a_al, ws_bytes - a_al, &o);
+    if (r != HOMG_OK) { homg_destroy(outer); return r; }
+    outer->inner = inner;
+    *out = outer;
+    return HOMG_OK;
+}
+
+static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, int levels, homg_stencil st,
+                              homg_dtype dt, void* ws, size_t ws_bytes, const homg_options* opt) {
     *out = nullptr;
     Plan P;
     std::string why;
@@ -195,6 +230,11 @@ homg_status homg_set_coefficient(homg_solver* s, const void* k, int on_device) {
     if (r != HOMG_OK) return r;
     CU(s, exec_sample_coef(s, s->stream));
     s->have_coef = true;
+    if (s->inner) {                                    // the correction cycle uses k rounded to fp32
+        CU(s, exec_cvt_coef_to_inner(s, s->stream));
+        CU(s, exec_sample_coef(s->inner, s->stream));
+        s->inner->have_coef = true;
+    }
     return reset_history(s);
 }
 
@@ -270,6 +310,7 @@ homg_status homg_profile_cycles(homg_solver* s, int n, double* ms_by_tag, int* l
     if (!s) return HOMG_EINVAL;
     if (!ms_by_tag || !launches_by_tag || !bytes_by_tag || cap < HOMG_TAG_COUNT) return set_err(s, HOMG_EINVAL, "profile arrays too small");
     if (!s->have_rhs || (s->var && !s->have_coef)) return set_err(s, HOMG_ESTATE, "profile before set_rhs / set_coefficient");
+    if (s->inner) return set_err(s, HOMG_ESTATE, "homg_profile_cycles is not available in mixed precision");
     for (int i = 0; i < cap; ++i) { ms_by_tag[i] = 0.0; launches_by_tag[i] = 0; bytes_by_tag[i] = 0.0; }
     CU(s, exec_prepare(s));
     for (int c = 0; c < n; ++c) CU(s, exec_cycle_profiled(s, s->stream, ms_by_tag, launches_by_tag, bytes_by_tag));
@@ -286,6 +327,7 @@ const char* homg_tag_name(int tag) {
 
 int homg_get_schedule(const homg_solver* s, int* lv, int* it, int cap) {
     if (!s) return -1;
+    if (s->inner) s = s->inner;
     int n = int(s->sched_lv.size());
     for (int i = 0; i < n && i < cap; ++i) {
         if (lv) lv[i] = s->sched_lv[i];
@@ -313,6 +355,7 @@ double homg_compulsory_bytes_per_cycle(const homg_solver* s, double* bytes_by_ta
 
 void homg_destroy(homg_solver* s) {
     if (!s) return;
+    if (s->inner) homg_destroy(s->inner);
     drop_graph(s);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->prog_dev) cudaFree(s->prog_dev);

@@ -952,6 +952,7 @@ cudaError_t exec_init(homg_solver* s) {
 }
 
 cudaError_t exec_prepare(homg_solver* s) {
+    if (s->inner) return exec_prepare(s->inner);                 // the outer problem has no coarse levels
     if (s->prog_ready || s->vcycle || s->literal) return cudaSuccess;       // the V-cycle has no coarse program
     Rec P{s, s->stream};
     P.plan = true;
@@ -967,7 +968,46 @@ cudaError_t exec_prepare(homg_solver* s) {
     return cudaSuccess;
 }
 
+// Mixed-precision outer cycle (the restart is a defect-correction loop):
+// `s` is the fp64 outer problem (one level: u, f, r), s->inner the fp32 hierarchy.  r = f - A u and its norm
+// in fp64 (K_res), r rounded to fp32 = the inner right-hand side, ONE fp32 HOMG cycle from e = 0, u += e in fp64.
+template <int ND>
+cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st) {
+    homg_solver* in = s->inner;
+    Rec R{s, st};
+    if (s->var) rec_norm<double, ND, true>(R, true, true, false);
+    else rec_norm<double, ND, false>(R, true, true, false);
+    const LevelGeom& go = s->L[0].g;
+    const LevelGeom& gi = in->L[0].g;
+    klaunch(R, k_cvt_pad<float, double, ND, false>, grd(gi), blk(), 0, gi, go, (const double*)s->L[0].gsrc, (float*)in->f);
+    R.check(TAG_OTHER);
+    R.acct(0, 1.5, TAG_OTHER);
+    cudaMemsetAsync(in->u, 0, in->L[0].n_alloc * sizeof(float), st);
+    R.check(TAG_OTHER);
+    R.acct(0, 0.5, TAG_OTHER);
+    Rec Ri{in, st};
+    HOMG_DISPATCH(in, rec_cycle, Ri);
+    klaunch(R, k_cvt_pad<double, float, ND, true>, grd(go), blk(), 0, go, gi, (const float*)in->u, (double*)s->u);
+    R.check(TAG_OTHER);
+    R.acct(0, 2.5, TAG_OTHER);
+    s->launches_per_cycle = R.launches + Ri.launches;
+    s->bytes_cycle_all = R.bytes_all + Ri.bytes_all;
+    s->bytes_cycle_l0 = R.bytes_l0 + Ri.bytes_l0;
+    for (int t = 0; t < TAG_COUNT; ++t) s->comp_by_tag[t] = R.comp_tag[t] + Ri.comp_tag[t];
+    return R.err != cudaSuccess ? R.err : Ri.err;
+}
+
+cudaError_t exec_cvt_coef_to_inner(homg_solver* s, cudaStream_t st) {
+    homg_solver* in = s->inner;
+    Rec R{s, st};
+    klaunch(R, k_cvt_pad<float, double, 3, false>, grd(in->L[0].g), blk(), 0, in->L[0].g, s->L[0].g, (const double*)s->L[0].k,
+            (float*)in->L[0].k);
+    R.check(TAG_OTHER);
+    return R.err;
+}
+
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
+    if (s->inner) return s->ndim == 2 ? cycle_mixed<2>(s, st) : cycle_mixed<3>(s, st);
     Rec R{s, st};
     if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
     else if (s->literal) HOMG_DISPATCH(s, rec_literal, R);

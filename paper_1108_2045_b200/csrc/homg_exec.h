@@ -32,6 +32,8 @@ cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_t
                                 double* bytes_by_tag);
 // ||f - A u||^2 of the current u -> *s->scalar (no history entry).
 cudaError_t exec_norm_only(homg_solver* s, cudaStream_t st);
+// mixed precision: nodal k of the fp64 outer problem -> fp32 k of the inner hierarchy (level 0)
+cudaError_t exec_cvt_coef_to_inner(homg_solver* s, cudaStream_t st);
 // k_m = k_{m-1} sampled at even nodes, m = 1..M.
 cudaError_t exec_sample_coef(homg_solver* s, cudaStream_t st);
 // dense C-order device array <-> padded level-0 array.

@@ -339,6 +339,17 @@ __global__ void k_unpack(LevelGeom g, const T* __restrict__ padded, T* __restric
     dense[((long long)z * g.ny + y) * g.nx + x] = padded[lidx(g, x, y, z)];
 }
 
+// mixed-precision outer loop: padded array of one precision -> padded array of another
+// (the row pitches differ), dst = TO(src) or dst += TO(src); one thread per node incl. the boundary
+template <class TO, class FROM, int ND, bool ADD>
+__global__ void k_cvt_pad(LevelGeom gto, LevelGeom gfrom, const FROM* __restrict__ src, TO* __restrict__ dst) {
+    pdl_start();
+    HOMG_NODE_XYZ(gto);
+    const long long d = lidx(gto, x, y, z);
+    const TO v = TO(src[lidx(gfrom, x, y, z)]);
+    dst[d] = ADD ? dst[d] + v : v;
+}
+
 // S0: face coefficients of one level from its nodal k (R11); 0 where the + neighbour does not exist
 template <class T, int ND>
 __global__ void k_faces(LevelGeom g, const T* __restrict__ k, T* __restrict__ fz, T* __restrict__ fy, T* __restrict__ fx) {

@@ -20,7 +20,7 @@ DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
 SYMBOLS = [
     "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
     "homg_set_coefficient", "homg_cycle", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
-    "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
+    "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_workspace_bytes_mixed", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
 ]
 
 
@@ -30,7 +30,7 @@ class HomgOptions(C.Structure):
         ("sched_levels", C.POINTER(C.c_int)), ("sched_iters", C.POINTER(C.c_int)), ("sched_len", C.c_int),
         ("coarse_threshold_nodes", C.c_int), ("use_graph", C.c_int), ("history_cap", C.c_int),
         ("tiled_min_nodes", C.c_int), ("march_chunk", C.c_int),
-        ("cuda_stream", C.c_void_p), ("cycle", C.c_int), ("v_eta1", C.c_int), ("v_eta2", C.c_int),
+        ("cuda_stream", C.c_void_p), ("cycle", C.c_int), ("v_eta1", C.c_int), ("v_eta2", C.c_int), ("mixed", C.c_int),
     ]
 
 
@@ -55,6 +55,7 @@ def lib():
         i64p = C.POINTER(C.c_int64)
         L.homg_default_options.argtypes = [C.POINTER(HomgOptions)]; L.homg_default_options.restype = None
         L.homg_workspace_bytes.argtypes = [i, i64p, i, i, i]; L.homg_workspace_bytes.restype = C.c_size_t
+        L.homg_workspace_bytes_mixed.argtypes = [i, i64p, i, i]; L.homg_workspace_bytes_mixed.restype = C.c_size_t
         L.homg_create.argtypes = [C.POINTER(vp), i, i64p, i, i, i, vp, C.c_size_t, C.POINTER(HomgOptions)]
         L.homg_create.restype = i
         for name in ("homg_set_rhs", "homg_set_initial_guess", "homg_set_coefficient", "homg_get_solution"):
@@ -98,7 +99,7 @@ class Solver:
 
     def __init__(self, dims, levels, stencil, dtype, omega=0.0, h=0.0, max_iters=0, schedule=HOMG_SCHED_C,
                  sched=None, coarse_threshold_nodes=0, use_graph=-1, history_cap=0, tiled_min_nodes=0,
-                 march_chunk=0, device="cuda:0", stream=None, vcycle=None, literal=False):
+                 march_chunk=0, device="cuda:0", stream=None, vcycle=None, literal=False, mixed=False):
         import torch
         self._torch = torch
         self.dims = tuple(int(x) for x in dims)
@@ -118,6 +119,8 @@ class Solver:
             o.cycle, o.v_eta1, o.v_eta2 = 1, int(vcycle[0]), int(vcycle[1])
         if literal:                                 # the paper's whole-grid iteration (Algorithm L)
             o.cycle = 2
+        if mixed:                                   # fp64 u, f, residual; the correction cycle in fp32
+            o.mixed = 1
         self._keep = None
         if sched is not None:
             lv, it = sched
@@ -127,10 +130,13 @@ class Solver:
         with torch.cuda.device(self.device):
             st = stream if stream is not None else torch.cuda.current_stream(self.device)
             o.cuda_stream = C.c_void_p(st.cuda_stream)
-            need = L.homg_workspace_bytes(len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil], DTYPES[dtype])
+            if mixed:
+                need = L.homg_workspace_bytes_mixed(len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil])
+            else:
+                need = L.homg_workspace_bytes(len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil], DTYPES[dtype])
             if need == 0:
                 raise HomgError(HOMG_EINVAL, L.homg_last_error(None).decode())
-            need += max(0, int(history_cap) - 4096) * 8 + 256
+            need += (2 if mixed else 1) * (max(0, int(history_cap) - 4096) * 8 + 256)
             self.workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
             rc = L.homg_create(C.byref(self.handle), len(self.dims), _dims(self.dims), self.levels, STENCILS[stencil],
                                DTYPES[dtype], C.c_void_p(self.workspace.data_ptr()), need, C.byref(o))

@@ -331,3 +331,38 @@ def test_full_size_first_cycles_vs_oracle(orc, name, ncyc):
     u = us[-1]
     for ax in range(u.ndim):
         assert not np.any(np.take(u, [0, -1], axis=ax))
+
+
+# ---- mixed-precision outer loop vs the oracle's mixed loop: fp64 u, f, r; fp32 correction cycle ----
+@pytest.mark.parametrize("name,n", [("cfg2", 33), ("cfg2", 65), ("cfg1", 129), ("cfg5", 33), ("cfg5", 65)])
+def test_mixed_precision_mode(orc, name, n):
+    cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+    assert cfg.dtype == "f64"
+    inp = I.make_inputs(cfg)
+    ncyc = 8
+    us, norms, sched = run_gpu(cfg, inp, ncyc, mixed=True)
+    _, hist, onorms = orc.homg_mixed(inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, ncyc, k=inp["k"])
+    for c in range(ncyc):
+        err = np.max(np.abs(us[c] - hist[c])) / np.max(np.abs(hist[c]))
+        assert err <= 1e-12, f"{cfg.name} mixed: cycle {c}: {err:.3e}"
+    assert np.allclose(norms, onorms, rtol=1e-9)
+
+
+def test_mixed_precision_keeps_contracting_below_the_fp32_floor(orc):
+    """the fp64 outer residual keeps contracting where the pure fp32 solve stalls at its rounding floor."""
+    import dataclasses
+    cfg = I.scaled(I.CONFIGS["cfg2"], 65)
+    inp = I.make_inputs(cfg)
+    _, norms, _ = run_gpu(cfg, inp, 30, mixed=True)
+    assert norms[-1] <= 1e-12 * norms[0]
+    cfg32 = dataclasses.replace(cfg, dtype="f32")
+    inp32 = {k: (None if v is None else v.astype(np.float32)) for k, v in inp.items()}
+    _, n32, _ = run_gpu(cfg32, inp32, 30)
+    assert norms[-1] / norms[0] < 1e-3 * n32[-1] / n32[0]
+
+
+def test_mixed_precision_argument_checks():
+    _torch()
+    from paper_1108_2045_b200 import homg
+    with pytest.raises(homg.HomgError):
+        homg.Solver((33, 33, 33), 5, "poisson7", "f64", mixed=True, vcycle=(2, 1))

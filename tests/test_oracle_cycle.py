@@ -308,3 +308,38 @@ def test_golden_paper_L1(orc):
         u, _, _ = orc.homg("H", f, np.zeros((129, 129)), 7, 0.8, orc.schedule(0, 7, int(mi)), 1, keep_history=False)
         mine = np.abs(u - uex).sum() / np.abs(uex).sum()
         assert abs(mine - err) < 0.3 * err, (mi, mine, err)
+
+
+# ---- mixed-precision outer loop (the restart is a defect-correction loop) ----
+@pytest.mark.parametrize("shape,levels,omega,var", [((17, 17), 4, 0.8, False), ((9, 9, 9), 3, 6 / 7, False),
+                                                    ((9, 9, 9), 3, 6 / 7, True), ((33, 33), 5, 0.8, False)])
+def test_mixed_precision_reaches_the_fp64_fixed_point(orc, shape, levels, omega, var):
+    """fp64 residual + fp32 correction cycle converges to the dense-LU solution to fp64 accuracy, where the pure
+    fp32 solve stalls at its rounding floor — pins the outer loop (residual in fp64, u += e in fp64)."""
+    rng = np.random.default_rng(5)
+    f = rng.standard_normal(shape)
+    k = np.exp(rng.uniform(-1, 1, shape)) if var else None
+    sched = orc.schedule(0, levels, 4)
+    ud = orc.dense_solve(f, k=k)
+    um, _, nm = orc.homg_mixed(f, np.zeros(shape), levels, omega, sched, 120, k=k, keep_history=False)
+    assert np.abs(um - ud).max() <= 1e-11 * np.abs(ud).max()
+    assert nm[-1] < 1e-10 * nm[0]
+    u32, _, n32 = orc.homg("H", f.astype(np.float32), np.zeros(shape, np.float32), levels, omega, sched, 120,
+                           k=None if k is None else k.astype(np.float32), keep_history=False)
+    assert np.abs(u32 - ud).max() > 1e-8 * np.abs(ud).max()          # the fp32 floor the mixed loop removes
+
+
+def test_mixed_precision_contracts_like_fp64(orc):
+    """per-cycle residual factors of the mixed loop equal the fp64 cycle's to 3 digits while the residual is above
+    the fp32 resolution of one cycle; the first cycle equals the fp32 cycle on the rounded right-hand side."""
+    shape, levels, omega = (33, 33, 33), 5, 6 / 7
+    rng = np.random.default_rng(6)
+    f = rng.standard_normal(shape)
+    sched = orc.schedule(0, levels, 4)
+    _, _, n64 = orc.homg("H", f, np.zeros(shape), levels, omega, sched, 8, keep_history=False)
+    um, hist, nm = orc.homg_mixed(f, np.zeros(shape), levels, omega, sched, 8)
+    for c in range(1, 8):
+        assert abs(nm[c] / nm[c - 1] - n64[c] / n64[c - 1]) <= 2e-3 * n64[c] / n64[c - 1], c
+    # from u = 0 the first residual is f itself: cycle 1 == one fp32 cycle on fl32(f), added in fp64
+    u1, _, _ = orc.homg("H", f.astype(np.float32), np.zeros(shape, np.float32), levels, omega, sched, 1, keep_history=False)
+    assert np.array_equal(hist[0], u1.astype(np.float64))
