@@ -245,7 +245,9 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
         const bool fin = own && (STEADY || q >= 2 * NS);
         Pack<T> uu;
         if (fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
-        if (fin && a) {                                            // S3e operands: into L1 now (no registers), read after the stages
+        // (a visit that starts with interpolate+correct is a level-0 visit: no S3e bookkeeping, no v^{NS-1}, v^{NS-2})
+        constexpr bool BOOK = !INTERP;
+        if (BOOK && fin && a) {                                    // S3e operands: into L1 now (no registers), read after the stages
             asm volatile("prefetch.global.L1 [%0];" ::"l"(v0 + cF));
             if (d0) asm volatile("prefetch.global.L1 [%0];" ::"l"(d0 + cF));
             if (!a_assign) asm volatile("prefetch.global.L1 [%0];" ::"l"(a + cF));
@@ -267,7 +269,7 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
             gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
         };
         // (3-D: one CTA of 512 threads per SM leaves 128 registers per thread; fetching ahead spills there)
-        constexpr bool AHEAD = ND == 2;
+        constexpr bool AHEAD = ND == 2 || INTERP;
         Pack<T> dnN, upN, gvN;
         T elN = T(0), erN = T(0);
         if (AHEAD) fetch(1, dnN, upN, gvN, elN, erN);
@@ -303,13 +305,13 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
                 for (int j = 0; j < VEC; ++j) out.v[j] = T(0);
             }
             if (s < NS) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
-            if (s == NS - 2 && s >= 1 && o2 != nullptr && own && (STEADY || (q >= 2 * NS - 2 && q <= nsteps - 3)))
+            if (BOOK && s == NS - 2 && s >= 1 && o2 != nullptr && own && (STEADY || (q >= 2 * NS - 2 && q <= nsteps - 3)))
                 *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * mstride) = out;
-            if (s == NS - 1 && s >= 1 && o1 != nullptr && own && (STEADY || (q >= 2 * NS - 1 && q <= nsteps - 2)))
+            if (BOOK && s == NS - 1 && s >= 1 && o1 != nullptr && own && (STEADY || (q >= 2 * NS - 1 && q <= nsteps - 2)))
                 *reinterpret_cast<Pack<T>*>(o1 + cF + mstride) = out;
             if (s == NS && fin) {
                 if (o0) *reinterpret_cast<Pack<T>*>(o0 + cF) = out;
-                if (a) {                                           // S3e: a (+)= d0 + v^{NS-1} - v^0
+                if (BOOK && a) {                                   // S3e: a (+)= d0 + v^{NS-1} - v^0
                     Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(v0 + cF), aa;
                     if (d0) dd = *reinterpret_cast<const Pack<T>*>(d0 + cF);
                     if (!a_assign) aa = *reinterpret_cast<const Pack<T>*>(a + cF);
