@@ -269,8 +269,12 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
     int mc = s->march_chunk > 0 ? std::min(s->march_chunk, interior) : (interior + best - 1) / best;
     const int nch = (interior + mc - 1) / mc;
     dim3 grid(tx, ND == 3 ? ty : nch, ND == 3 ? nch : 1);
-    klaunch(R, k_visit<T, ND, NS, INTERP>, grid, TL::NT, visit_smem_bytes<T, ND, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
-            make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+    if (!INTERP && (a || o1 || o2))
+        klaunch(R, k_visit<T, ND, NS, false, true>, grid, TL::NT, visit_smem_bytes<T, ND, NS, false>(), tm_in, tm_ac, tm_g, g,
+                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+    else
+        klaunch(R, k_visit<T, ND, NS, INTERP, false>, grid, TL::NT, visit_smem_bytes<T, ND, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
+                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
 }
 
 template <class T, int ND, bool INTERP>
@@ -905,10 +909,13 @@ cudaError_t set_attr_coarse() {
 
 template <class T, int ND, int NS>
 cudaError_t set_attr_visit1() {
-    cudaError_t e = cudaFuncSetAttribute(k_visit<T, ND, NS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_visit<T, ND, NS, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          visit_smem_bytes<T, ND, NS, false>());
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_visit<T, ND, NS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    e = cudaFuncSetAttribute(k_visit<T, ND, NS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             visit_smem_bytes<T, ND, NS, false>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_visit<T, ND, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 visit_smem_bytes<T, ND, NS, true>());
 }
 template <class T, int NS>

@@ -76,7 +76,9 @@ __host__ __device__ constexpr int visit_smem_bytes() {
 // o0 / o1 / o2 : v^NS, v^{NS-1}, v^{NS-2} (each may be null);  a, a_assign, d0, v0, u : as k_relax
 // grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior planes);  2-D: (x tiles, y chunks)
 // ("z" / "plane" below = the marching axis: z in 3-D, y in 2-D)
-template <class T, int ND, int NS, bool INTERP>
+// BOOK: the visit of a level >= 1 (S3e bookkeeping, v^{NS-1} / v^{NS-2} stored, no u); otherwise a level-0
+// visit (u optional, nothing else) — two compiled variants so that neither carries the other's registers.
+template <class T, int ND, int NS, bool INTERP, bool BOOK>
 __global__ void __launch_bounds__(VisitTile<T, ND, NS>::NT, VisitTile<T, ND, NS>::CTAS)
 k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
          const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
@@ -244,9 +246,8 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
         // so that its HBM latency hides behind the arithmetic
         const bool fin = own && (STEADY || q >= 2 * NS);
         Pack<T> uu;
-        if (fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
-        // (a visit that starts with interpolate+correct is a level-0 visit: no S3e bookkeeping, no v^{NS-1}, v^{NS-2})
-        constexpr bool BOOK = !INTERP;
+        if (!BOOK && fin && u) uu = *reinterpret_cast<const Pack<T>*>(u + cF);
+        static_assert(!(INTERP && BOOK), "interpolate+correct is fused on level 0 only");
         if (BOOK && fin && a) {                                    // S3e operands: into L1 now (no registers), read after the stages
             asm volatile("prefetch.global.L1 [%0];" ::"l"(v0 + cF));
             if (d0) asm volatile("prefetch.global.L1 [%0];" ::"l"(d0 + cF));
@@ -269,7 +270,7 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
             gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
         };
         // (3-D: one CTA of 512 threads per SM leaves 128 registers per thread; fetching ahead spills there)
-        constexpr bool AHEAD = ND == 2 || INTERP;
+        constexpr bool AHEAD = ND == 2 || !BOOK;
         Pack<T> dnN, upN, gvN;
         T elN = T(0), erN = T(0);
         if (AHEAD) fetch(1, dnN, upN, gvN, elN, erN);
@@ -322,7 +323,7 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
                     }
                     *reinterpret_cast<Pack<T>*>(a + cF) = aa;
                 }
-                if (u) {                                           // S4: u += v^NS
+                if (!BOOK && u) {                                  // S4: u += v^NS
 #pragma unroll
                     for (int j = 0; j < VEC; ++j) uu.v[j] += out.v[j];
                     *reinterpret_cast<Pack<T>*>(u + cF) = uu;
