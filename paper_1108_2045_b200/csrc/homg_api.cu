@@ -107,6 +107,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (r != HOMG_OK) return r;
     r = create_one(&inner, ndim, dims, levels, st, HOMG_F32, static_cast<char*>(ws) + a_al, ws_bytes - a_al, &o);
     if (r != HOMG_OK) { homg_destroy(outer); return r; }
+    inner->given_g0 = true;
     outer->inner = inner;
     *out = outer;
     return HOMG_OK;

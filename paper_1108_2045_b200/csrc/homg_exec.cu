@@ -32,6 +32,7 @@ struct Rec {                 // bookkeeping while recording
     int last_tag = TAG_OTHER;
     double bytes_tag[TAG_COUNT] = {};         // algorithmic bytes per kernel class (per sweep)
     double comp_tag[TAG_COUNT] = {};          // compulsory bytes per kernel class (what the launch must move)
+    bool skip_s1 = false;                     // mixed precision: g_0 is given (the rounded fp64 residual), no S1 here
     const void* g_override = nullptr;         // V-cycle, level 0: the sweeps' right-hand side is f, not g_0
     const void* u_override = nullptr;         // V-cycle: the residual is taken of this iterate instead of u
     bool plan = false;                        // planning pass: build the coarse program, launch nothing
@@ -389,7 +390,7 @@ void rec_cycle(Rec& R) {
     auto flush = [&]() { flush_run<T, ND, VAR>(R); };
 
     // S1: r = f - A u, ||r||^2 -> history
-    const bool have_g1 = rec_norm<T, ND, VAR>(R, true, true, true);
+    const bool have_g1 = R.skip_s1 ? false : rec_norm<T, ND, VAR>(R, true, true, true);
     // S2: nested restriction g_m = P g_{m-1}
     for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
         if (small(m)) {
@@ -963,6 +964,7 @@ cudaError_t exec_prepare(homg_solver* s) {
     if (s->prog_ready || s->vcycle || s->literal) return cudaSuccess;       // the V-cycle has no coarse program
     Rec P{s, s->stream};
     P.plan = true;
+    P.skip_s1 = s->given_g0;
     HOMG_DISPATCH(s, rec_cycle, P);
     if (P.err != cudaSuccess) return P.err;
     if (!P.prog.empty()) {
@@ -986,15 +988,18 @@ cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st) {
     else rec_norm<double, ND, false>(R, true, true, false);
     const LevelGeom& go = s->L[0].g;
     const LevelGeom& gi = in->L[0].g;
-    klaunch(R, k_cvt_pad<float, double, ND, false>, grd(gi), blk(), 0, gi, go, (const double*)s->L[0].gsrc, (float*)in->f);
+    // g_0 of the inner hierarchy = fl32(r): the inner cycle's own S1 would compute f_in - A 0 = f_in, so it is skipped
+    const dim3 g4((go.nx + 127) / 128, (go.ny + 7) / 8, go.nz);
+    klaunch(R, k_cvt4<ND, false>, g4, blk(), 0, go, gi, (double*)s->L[0].gsrc, (float*)in->L[0].gsrc);
     R.check(TAG_OTHER);
     R.acct(0, 1.5, TAG_OTHER);
     cudaMemsetAsync(in->u, 0, in->L[0].n_alloc * sizeof(float), st);
     R.check(TAG_OTHER);
     R.acct(0, 0.5, TAG_OTHER);
     Rec Ri{in, st};
+    Ri.skip_s1 = in->given_g0;
     HOMG_DISPATCH(in, rec_cycle, Ri);
-    klaunch(R, k_cvt_pad<double, float, ND, true>, grd(go), blk(), 0, go, gi, (const float*)in->u, (double*)s->u);
+    klaunch(R, k_cvt4<ND, true>, g4, blk(), 0, go, gi, (double*)s->u, (float*)in->u);
     R.check(TAG_OTHER);
     R.acct(0, 2.5, TAG_OTHER);
     s->launches_per_cycle = R.launches + Ri.launches;

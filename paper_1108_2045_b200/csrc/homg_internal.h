@@ -76,6 +76,7 @@ struct homg_solver {
     bool fuse_first = true;          // fused interpolate+correct+relax first sweep (HOMG_FUSE_FIRST=0 disables)
     bool fuse_first_var = false;     // ... for the variable-coefficient stencil: measured slower than deliver + sweep
                                      // (cfg5: 535 us vs 64 + 190 us), off unless HOMG_FUSE_FIRST_VAR=1
+    bool given_g0 = false;           // this is the inner hierarchy of a mixed-precision solver: g_0 is written by the outer loop
     homg_solver* inner = nullptr;    // mixed precision: this is the fp64 outer problem (1 level), inner the
                                      // fp32 hierarchy that runs the correction cycle; owned by this object
     bool literal = false;            // paper-literal whole-grid iteration, Algorithm L

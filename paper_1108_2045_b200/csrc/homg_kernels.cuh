@@ -350,6 +350,29 @@ __global__ void k_cvt_pad(LevelGeom gto, LevelGeom gfrom, const FROM* __restrict
     dst[d] = ADD ? dst[d] + v : v;
 }
 
+// the same for the two level-0 passes of every mixed cycle, four x nodes per thread (rows of both arrays
+// start 128-B aligned): r32 = float(r64)  /  u64 += double(e32)
+template <int ND, bool ADD>
+__global__ void __launch_bounds__(256)
+k_cvt4(LevelGeom g64, LevelGeom g32, double* __restrict__ d64, float* __restrict__ f32) {
+    pdl_start();
+    const int x = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g64.nx || y >= g64.ny || z >= g64.nz) return;
+    double2* p64 = reinterpret_cast<double2*>(d64 + lidx(g64, x, y, z));
+    float4* p32 = reinterpret_cast<float4*>(f32 + lidx(g32, x, y, z));
+    if (ADD) {
+        const float4 e = *p32;
+        double2 a = p64[0], b = p64[1];
+        a.x += double(e.x); a.y += double(e.y); b.x += double(e.z); b.y += double(e.w);
+        p64[0] = a; p64[1] = b;
+    } else {
+        const double2 a = p64[0], b = p64[1];
+        *p32 = make_float4(float(a.x), float(a.y), float(b.x), float(b.y));
+    }
+}
+
 // S0: face coefficients of one level from its nodal k (R11); 0 where the + neighbour does not exist
 template <class T, int ND>
 __global__ void k_faces(LevelGeom g, const T* __restrict__ k, T* __restrict__ fz, T* __restrict__ fy, T* __restrict__ fx) {
