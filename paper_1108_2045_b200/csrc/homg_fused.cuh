@@ -150,22 +150,28 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
     // VAR: faces of this thread's nodes; the z- face of a plane is the z+ face of the one before
     const bool kok = VAR && row_ok && row_int;
-    Pack<T> fzm;
-    if (kok) fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
+    Pack<T> fzm, nfz, nfym, nfyp, nfx;
+    T nfxl = T(0);
+    auto fetch_faces = [&](const long long cc) {
+        nfz = *reinterpret_cast<const Pack<T>*>(kf.z + cc);
+        nfym = *reinterpret_cast<const Pack<T>*>(kf.y + cc - g.px);
+        nfyp = *reinterpret_cast<const Pack<T>*>(kf.y + cc);
+        nfx = *reinterpret_cast<const Pack<T>*>(kf.x + cc);
+        if (x > 0) nfxl = kf.x[cc - 1];
+    };
+    if (kok) {
+        fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
+        fetch_faces(c);
+    }
     // one plane; K = (i-1) mod 4 is a compile-time constant so that every stage address is an immediate
     auto step = [&](auto KC, const int i) {
         constexpr int K = decltype(KC)::value;
         constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
+        // faces of this plane were fetched one step ago; those of the next plane (it exists: z+1 <= NM-1) now
+        const Pack<T> fzp = nfz, fym = nfym, fyp = nfyp, fxp = nfx;
+        const T fxl = nfxl;
+        if (kok) fetch_faces(c + mstride);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
-        Pack<T> fzp, fym, fyp, fxp;
-        T fxl = T(0);
-        if (kok) {
-            fzp = *reinterpret_cast<const Pack<T>*>(kf.z + c);
-            fym = *reinterpret_cast<const Pack<T>*>(kf.y + c - g.px);
-            fyp = *reinterpret_cast<const Pack<T>*>(kf.y + c);
-            fxp = *reinterpret_cast<const Pack<T>*>(kf.x + c);
-            if (x > 0) fxl = kf.x[c - 1];
-        }
         nxt = *reinterpret_cast<const Pack<T>*>(vs(sn) + voff);
         const T* vt = vs(sc);
         Pack<T> dn, up;
@@ -368,22 +374,28 @@ k_res_tma(const __grid_constant__ CUtensorMap tmu, const __grid_constant__ CUten
     long long c = (long long)ms * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
     // VAR: face coefficients straight from global memory (see k_relax_tma)
     const bool kok = VAR && x >= 0 && x < g.nx && row_int;
-    Pack<T> fzm;
-    if (kok) fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
+    Pack<T> fzm, nfz, nfym, nfyp, nfx;
+    T nfxl = T(0);
+    auto fetch_faces = [&](const long long cc) {
+        nfz = *reinterpret_cast<const Pack<T>*>(kf.z + cc);
+        nfym = *reinterpret_cast<const Pack<T>*>(kf.y + cc - g.px);
+        nfyp = *reinterpret_cast<const Pack<T>*>(kf.y + cc);
+        nfx = *reinterpret_cast<const Pack<T>*>(kf.x + cc);
+        if (x > 0) nfxl = kf.x[cc - 1];
+    };
+    if (kok) {
+        fzm = *reinterpret_cast<const Pack<T>*>(kf.z + c - mstride);
+        fetch_faces(c);
+    }
     auto step = [&](auto KC, const int i) {
         constexpr int K = decltype(KC)::value;
         const int z = ms - 1 + i;
         constexpr int sn = (K + 2) & (TL::NST - 1), sc = (K + 1) & (TL::NST - 1);
+        // faces of this plane were fetched one step ago; those of the next plane (it exists: z+1 <= NM-1) now
+        const Pack<T> fzp = nfz, fym = nfym, fyp = nfyp, fxp = nfx;
+        const T fxl = nfxl;
+        if (kok) fetch_faces(c + mstride);
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
-        Pack<T> fzp, fym, fyp, fxp;
-        T fxl = T(0);
-        if (kok) {
-            fzp = *reinterpret_cast<const Pack<T>*>(kf.z + c);
-            fym = *reinterpret_cast<const Pack<T>*>(kf.y + c - g.px);
-            fyp = *reinterpret_cast<const Pack<T>*>(kf.y + c);
-            fxp = *reinterpret_cast<const Pack<T>*>(kf.x + c);
-            if (x > 0) fxl = kf.x[c - 1];
-        }
         nxt = *reinterpret_cast<const Pack<T>*>(us(sn) + voff);
         const T* vt = us(sc);
         Pack<T> dn, up;
