@@ -235,6 +235,25 @@ def test_kvisit_matches_per_sweep_kernels_bitwise(orc, monkeypatch, name, n, max
     assert np.array_equal(na, nb)
 
 
+@pytest.mark.parametrize("name,n,maxi,kind", [("cfg2", 65, 4, 0), ("cfg5", 33, 4, 0), ("cfg5", 65, 3, 1), ("cfg1", 129, 4, 0),
+                                              ("cfg3", 257, 2, 2), ("cfg4", 33, 4, 1), ("cfg1", 65, 3, 1)])
+def test_kmid_matches_per_sweep_kernels_bitwise(orc, monkeypatch, name, n, maxi, kind):
+    """K_mid (a whole visit of a mid-size level in one launch: block tiles in shared memory, halo of eta nodes
+    recomputed) is bit-identical to one k_relax launch per sweep: 2-D / 3-D, both dtypes, constant and variable
+    coefficient, eta = 2, 3, 4, level 0 as a mid level (u += e), schedules that revisit and move up from level 0;
+    and it matches the oracle."""
+    import dataclasses
+    cfg = dataclasses.replace(I.scaled(I.CONFIGS[name], n), max_iters=maxi, schedule=kind)
+    check_parity(cfg, 3, orc)
+    inp = I.make_inputs(cfg)
+    a, na, _ = run_gpu(cfg, inp, 3)
+    monkeypatch.setenv("HOMG_FUSE_MID", "0")
+    b, nb, _ = run_gpu(cfg, inp, 3)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert np.array_equal(na, nb)
+
+
 def test_variable_coefficient_fused_first_sweep(orc, monkeypatch):
     """k_relax_first for the variable-coefficient stencil (off by default: slower than deliver + sweep on cfg5)."""
     monkeypatch.setenv("HOMG_FUSE_FIRST_VAR", "1")
