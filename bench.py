@@ -131,6 +131,8 @@ def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False, mixed=False):
                     schedule=cfg.schedule, device=dev, vcycle=vcycle, literal=literal, mixed=mixed)
     tdt = torch.float64 if cfg.dtype == "f64" else torch.float32
     d = {k: (None if v is None else torch.from_numpy(v).to(dev)) for k, v in inp.items()}
+    if not inp["u0"].any():
+        d["u0"] = None          # the config's u0 = 0 is the library's default guess: set_initial_guess(None), no array
     if d["k"] is not None:
         s.set_coefficient(d["k"])
     s.set_rhs(d["f"])
@@ -317,7 +319,7 @@ def run_homg(args):
 
     # ---- e2e: host buffers through the C ABI ----
     hf = torch.from_numpy(inp["f"]).pin_memory()
-    hu0 = torch.from_numpy(inp["u0"]).pin_memory()
+    hu0 = torch.from_numpy(inp["u0"]).pin_memory() if inp["u0"].any() else None     # u0 = 0: the default guess, no upload
     hk = None if inp["k"] is None else torch.from_numpy(inp["k"]).pin_memory()
     hout = torch.empty(cfg.dims, dtype=hf.dtype).pin_memory()
 
@@ -359,7 +361,7 @@ def run_homg(args):
     peak, peak_src = peaks()
     comp, comp_total = s.compulsory_bytes_per_cycle()
     rl, shares = roofline_from_profile(prof, peak, peak_src, comp, cstar, cfg.name)
-    launches_step = s.launches_per_cycle() * cstar + 2 + 2          # + pack(u0) + norm-only pass (2 kernels)
+    launches_step = s.launches_per_cycle() * cstar + (2 if d["u0"] is not None else 0) + 2   # + pack(u0) (u0 = 0: a memset, not counted) + norm-only pass (2 kernels)
     bytes_cycle = s.bytes_per_cycle()
     clocks = sampler.stop()
 
@@ -381,7 +383,7 @@ def run_homg(args):
             "cycle_compulsory_gb": comp_total / 1e9,
             "cycle_compulsory_gbs": comp_total / (total_ms * 1e-3 / args.steps / cstar) / 1e9,
             "e2e": {"value": cfg.n_interior * n_e2e * world / e2e_s, "unit": UNIT, "ms_per_step": e2e_s / n_e2e * 1e3,
-                    "h2d_bytes_per_step": nbytes * (3 if hk is not None else 2), "d2h_bytes_per_step": nbytes + 8},
+                    "h2d_bytes_per_step": nbytes * (1 + (hk is not None) + (hu0 is not None)), "d2h_bytes_per_step": nbytes + 8},
             "gpu_launches": launches_step * args.steps, "roofline": rl, "kernels": shares, "clocks": clocks}
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:

@@ -132,7 +132,8 @@ HOMG_API homg_status homg_create(homg_solver** out, int ndim, const int64_t* dim
 /* Right-hand side f (Eq.1).  Resets the norm history. */
 HOMG_API homg_status homg_set_rhs(homg_solver* s, const void* f, int on_device);
 
-/* Initial guess u0 (default 0).  Resets the norm history. */
+/* Initial guess u0 (default 0).  u0 == NULL restores the default guess u = 0 on the device (no
+ * transfer; on_device is ignored), e.g. before solving again.  Resets the norm history. */
 HOMG_API homg_status homg_set_initial_guess(homg_solver* s, const void* u0, int on_device);
 
 /* Nodal coefficient k > 0 (HOMG_DIFFUSION7 only): sampled onto every level by

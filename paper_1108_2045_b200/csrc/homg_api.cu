@@ -148,7 +148,6 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST_VAR")) s->fuse_first_var = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
-    if (const char* ev = std::getenv("HOMG_FUSE_MID")) s->fuse_mid = std::atoi(ev) != 0;
     s->vcycle = o.cycle == HOMG_CYCLE_V;
     s->literal = o.cycle == HOMG_CYCLE_LITERAL;
     s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;
@@ -218,7 +217,10 @@ homg_status homg_set_rhs(homg_solver* s, const void* f, int on_device) {
 
 homg_status homg_set_initial_guess(homg_solver* s, const void* u0, int on_device) {
     if (!s) return HOMG_EINVAL;
-    if (!u0) return set_err(s, HOMG_EINVAL, "u0 is null");
+    if (!u0) {                                         // the default guess u0 = 0: no transfer, one memset
+        CU(s, cudaMemsetAsync(s->u, 0, s->L[0].n_alloc * size_t(s->dtype), s->stream));
+        return reset_history(s);
+    }
     homg_status r = load_dense(s, u0, on_device, s->u, 1);
     if (r != HOMG_OK) return r;
     return reset_history(s);

@@ -12,7 +12,6 @@
 #include "homg_coarse.cuh"
 #include "homg_first.cuh"
 #include "homg_visit.cuh"
-#include "homg_mid.cuh"
 #include "homg_moves.cuh"
 #include "homg_literal.cuh"
 
@@ -285,20 +284,6 @@ void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* a
     if (ns == 2) launch_visit<T, ND, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
     else if (ns == 3) launch_visit<T, ND, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
     else launch_visit<T, ND, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
-}
-
-// K_mid: all eta sweeps of a visit on a mid-size level in one launch (homg_mid.cuh)
-template <class T, int ND, bool VAR>
-void launch_visit_mid(Rec& R, int t, int eta, const T* vin, T* o0, T* o1, T* o2, T* a, int a_assign, const T* d0,
-                      const T* v0, T* u) {
-    homg_solver* s = R.s;
-    Level& Lt = s->L[t];
-    using TL = MidTile<T, ND>;
-    const LevelGeom& g = Lt.g;
-    const int ow = TL::TX - 2 * eta;                 // TX = TY = TZ (3-D)
-    dim3 grid((g.nx + ow - 1) / ow, (g.ny + ow - 1) / ow, ND == 3 ? (g.nz + ow - 1) / ow : 1);
-    klaunch(R, k_visit_mid<T, ND, VAR>, grid, dim3(TL::NT, 1, 1), size_t(TL::SMEM), g, make_coef<T>(s, t), vin,
-            (const T*)(R.g_override ? R.g_override : Lt.gsrc), faces<T>(Lt), eta, o0, o1, o2, a, a_assign, d0, v0, u);
 }
 
 // launches the pending run of coarse-level operations as ONE cluster (K_coarse)
@@ -667,37 +652,6 @@ void rec_cycle(Rec& R) {
             cur = t;
             continue;
         }
-        // a mid-size level (neither one CTA's nor the tiled kernels'): the whole visit is ONE launch of K_mid
-        if (!small(t) && !tiled(s, t) && s->fuse_mid && eta >= 2 && eta <= MidTile<T, ND>::MAX_ETA) {
-            flush();
-            // where v^eta, v^{eta-1}, v^{eta-2} go: never the input (other CTAs read its halo).  Level 0 has
-            // three buffers: v^{eta-2} is not kept there (S3c never needs the dp of the finest level).
-            int b0 = -1, b1 = -1, b2 = -1;
-            for (int b = 0; b < Lt.nrot; ++b) {
-                if (b == v0) continue;
-                if (b0 < 0) b0 = b; else if (b1 < 0) b1 = b; else if (b2 < 0) b2 = b;
-            }
-            if (eta < 3 || t == 0) b2 = -1;
-            const bool book = t >= 1, addu = vi == nv - 1;
-            if (!R.plan)
-                launch_visit_mid<T, ND, VAR>(R, t, eta, rotp<T>(Lt, v0), rotp<T>(Lt, b0), rotp<T>(Lt, b1), rotp<T>(Lt, b2),
-                                             book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, (book && have_d0) ? (const T*)Lt.d0 : nullptr,
-                                             rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
-            const int tag = t == 0 ? TAG_VISIT0 : TAG_VISIT;
-            R.check(tag);
-            {
-                const double bk = book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) : 0.0;
-                const double fc = VAR ? 3.0 : 0.0;
-                const double comp = 2.0 + fc + 2.0 + (b2 >= 0 ? 1.0 : 0.0) + bk + (addu ? 2.0 : 0.0);
-                const double alg = (3.0 + fc) * eta + (addu ? 2.0 : 0.0) + bk + (book ? 1.0 : 0.0);
-                R.acct2(t, alg, comp, tag);
-            }
-            if (t >= 1) a_zero[t] = 0;
-            Lt.vk = b0; Lt.vkm1 = b1; Lt.vkm2 = (eta == 2 && t >= 1) ? v0 : b2; Lt.e = b0; Lt.eta_last = eta;
-            dp_is_d0[t] = false;
-            cur = t;
-            continue;
-        }
         for (int it = 0; it < eta; ++it) {
             int out = -1;
             for (int b = 0; b < Lt.nrot; ++b)
@@ -948,11 +902,6 @@ cudaError_t set_attr() {
 }
 
 template <class T, int ND, bool VAR>
-cudaError_t set_attr_mid() {
-    return cudaFuncSetAttribute(k_visit_mid<T, ND, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, MidTile<T, ND>::SMEM);
-}
-
-template <class T, int ND, bool VAR>
 cudaError_t set_attr_coarse() {
     cudaError_t e = cudaFuncSetAttribute(k_coarse_run<T, ND, VAR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRelaxnSmemMax);
     if (e != cudaSuccess) return e;
@@ -995,12 +944,6 @@ cudaError_t exec_init(homg_solver* s) {
     if ((e = set_attr<double, 2, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, false>()) != cudaSuccess) return e;
     if ((e = set_attr<double, 3, true>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<float, 2, false>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<float, 3, false>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<float, 3, true>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<double, 2, false>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<double, 3, false>()) != cudaSuccess) return e;
-    if ((e = set_attr_mid<double, 3, true>()) != cudaSuccess) return e;
     if ((e = set_attr_coarse<float, 2, false>()) != cudaSuccess) return e;
     if ((e = set_attr_coarse<float, 3, false>()) != cudaSuccess) return e;
     if ((e = set_attr_coarse<float, 3, true>()) != cudaSuccess) return e;

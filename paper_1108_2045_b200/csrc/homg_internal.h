@@ -83,7 +83,6 @@ struct homg_solver {
     bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
     int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
-    bool fuse_mid = true;            // K_mid: a visit of a mid-size level in one launch (HOMG_FUSE_MID=0: one launch per sweep)
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create
     std::vector<int> sched_lv, sched_it;

@@ -159,6 +159,11 @@ class Solver:
         self._call_arr(lib().homg_set_rhs, f)
 
     def set_initial_guess(self, u0):
+        """u0 = None: the default guess u = 0 (homg_set_initial_guess with a null pointer)."""
+        if u0 is None:
+            with self._torch.cuda.device(self.device):
+                self._ck(lib().homg_set_initial_guess(self.handle, C.c_void_p(0), 0))
+            return
         self._call_arr(lib().homg_set_initial_guess, u0)
 
     def set_coefficient(self, k):
