@@ -102,6 +102,19 @@ void klaunch(Rec& R, K kern, dim3 grid, dim3 block, size_t smem, Args... args) {
 }
 inline dim3 d3(int x) { return dim3(x, 1, 1); }
 
+// resident CTAs per SM of a kernel at its launch configuration (asked of the runtime once per kernel): the
+// marching-axis chunk counts are chosen so that tiles x chunks fills whole waves of sm_count x this
+template <class K>
+int resident_ctas(K kern, int threads, size_t smem) {
+    static std::vector<std::pair<const void*, int>> cache;       // keyed by the kernel's address (one K per signature)
+    const void* key = reinterpret_cast<const void*>(kern);
+    for (auto& c : cache) if (c.first == key) return c.second;
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, smem) != cudaSuccess || n < 1) n = 1;
+    cache.push_back({key, n});
+    return n;
+}
+
 inline dim3 blk() { return dim3(32, 8, 1); }
 inline dim3 grd(const LevelGeom& g) { return dim3((g.nx + 31) / 32, (g.ny + 7) / 8, g.nz); }
 template <class T>
@@ -258,7 +271,10 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
     const int tx = (g.nx - 1 + TL::OX - 1) / TL::OX, ty = ND == 3 ? (g.ny - 1 + TL::OY - 1) / TL::OY : 1;
     const long long tiles = (long long)tx * ty;
     // chunks of the marching axis: pick the count that minimises waves x (planes per chunk + pipeline fill)
-    const long long slots = (long long)s->sm_count * TL::CTAS;
+    const bool bookv = !INTERP && (a || o1 || o2);
+    const int occ = bookv ? resident_ctas(k_visit<T, ND, NS, false, true>, TL::NT, visit_smem_bytes<T, ND, NS, false>())
+                          : resident_ctas(k_visit<T, ND, NS, INTERP, false>, TL::NT, visit_smem_bytes<T, ND, NS, INTERP>());
+    const long long slots = (long long)s->sm_count * occ;
     int best = 1;
     double bestc = 1e300;
     for (int nch = 1; nch <= 256 && nch <= interior; ++nch) {
@@ -270,7 +286,7 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
     int mc = s->march_chunk > 0 ? std::min(s->march_chunk, interior) : (interior + best - 1) / best;
     const int nch = (interior + mc - 1) / mc;
     dim3 grid(tx, ND == 3 ? ty : nch, ND == 3 ? nch : 1);
-    if (!INTERP && (a || o1 || o2))
+    if (bookv)
         klaunch(R, k_visit<T, ND, NS, false, true>, grid, TL::NT, visit_smem_bytes<T, ND, NS, false>(), tm_in, tm_ac, tm_g, g,
                 make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
     else
@@ -345,7 +361,8 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
         int mc = s->march_chunk;
         if (mc <= 0) {
-            long long nch = std::max<long long>(1, (long long)s->sm_count * 3 / std::max<long long>(tiles, 1));
+            const int occ = resident_ctas(k_res_tma<T, ND, VAR>, TL::NW * 32, res_smem_bytes<T, ND, VAR>());
+            long long nch = std::max<long long>(1, (long long)s->sm_count * occ / std::max<long long>(tiles, 1));
             mc = std::max(int((interior + nch - 1) / nch), 8);
         }
         mc = (mc + 1) & ~1;                                        // even: chunks start on odd planes
