@@ -78,8 +78,13 @@ __host__ __device__ constexpr int visit_smem_bytes() {
 // ("z" / "plane" below = the marching axis: z in 3-D, y in 2-D)
 // BOOK: the visit of a level >= 1 (S3e bookkeeping, v^{NS-1} / v^{NS-2} stored, no u); otherwise a level-0
 // visit (u optional, nothing else) — two compiled variants so that neither carries the other's registers.
+// CTAs per SM the register allocation aims at: 3-D one 512-thread CTA; 2-D (160 threads) four level-0 CTAs
+// (<= 96 registers) or three with the S3e bookkeeping
+template <int ND, bool BOOK>
+__host__ __device__ constexpr int visit_ctas() { return ND == 3 ? 1 : (BOOK ? 3 : 4); }
+
 template <class T, int ND, int NS, bool INTERP, bool BOOK>
-__global__ void __launch_bounds__(VisitTile<T, ND, NS>::NT, VisitTile<T, ND, NS>::CTAS)
+__global__ void __launch_bounds__(VisitTile<T, ND, NS>::NT, visit_ctas<ND, BOOK>())
 k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
          const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
          T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
