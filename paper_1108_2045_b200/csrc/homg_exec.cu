@@ -175,14 +175,14 @@ inline bool tiled(const homg_solver* s, int m) {
 
 // planes per CTA along the marching axis: as few chunks as fill the machine about once
 template <class T, int ND>
-int march_chunk(const homg_solver* s, const LevelGeom& g, int* nchunks) {
+int march_chunk(const homg_solver* s, const LevelGeom& g, int* nchunks, int occ = 4) {
     using TL = Tile<T, ND>;
     const int NM = ND == 3 ? g.nz : g.ny;
     const int interior = std::max(NM - 2, 1);
     long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
     int mc = s->march_chunk;
     if (mc <= 0) {
-        long long slots = (long long)s->sm_count * 4;
+        long long slots = (long long)s->sm_count * occ;
         long long nch = std::max<long long>(1, slots / std::max<long long>(tiles, 1));
         mc = int((interior + nch - 1) / nch);
         mc = std::max(mc, 8);
@@ -205,7 +205,7 @@ void launch_relax(Rec& R, int t, const T* vin, T* vout, T* a, int a_assign, cons
                   make_tmap<T, ND>(s, &tmg, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::SEG, ND == 3 ? TL::TY : 1);
         if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
         int nch = 1;
-        int mc = march_chunk<T, ND>(s, Lt.g, &nch);
+        int mc = march_chunk<T, ND>(s, Lt.g, &nch, resident_ctas(k_relax_tma<T, ND, VAR>, 256, relax_smem_bytes<T, ND, VAR>()));
         dim3 grid((Lt.g.nx - 1 + TL::TX - 1) / TL::TX, ND == 3 ? (Lt.g.ny - 1 + TL::TY - 1) / TL::TY : nch, ND == 3 ? nch : 1);
         if (u && t == 0) vout = nullptr;              // e_0 is dead after u += e_0: do not write it
         klaunch(R, k_relax_tma<T, ND, VAR>, grid, 256, relax_smem_bytes<T, ND, VAR>(), tmv, tmg, faces<T>(Lt), Lt.g, cf, vout, a, a_assign,
