@@ -162,6 +162,11 @@ NCU_TRAFFIC = {
     ("cfg4", "relax_l0"): (1.164186e9 + 0.509018e9, "profiles/r01b_ncu_full_cfg4.md"),
     ("cfg2", "visit_l0"): (43.483904e6 + 0.012800e6, "profiles/r01d_ncu_full_cfg2.md"),      # L2-resident (17 MB arrays)
     ("cfg2", "residual_l0"): (36.909056e6 + 0.042752e6, "profiles/r01d_ncu_full_cfg2.md"),
+    ("cfg3", "visit_l0"): (693.390848e6 + 235.526656e6, "profiles/r01e_ncu_full_cfg3.md"),
+    ("cfg3", "residual_l0"): (548.102656e6 + 302.414592e6, "profiles/r01e_ncu_full_cfg3.md"),
+    ("cfg5", "relax_l0"): (687.057920e6 + 121.797120e6, "profiles/r01e_ncu_full_cfg5.md"),
+    ("cfg5", "relax_l0_last"): (820.713472e6 + 122.384128e6, "profiles/r01e_ncu_full_cfg5.md"),
+    ("cfg5", "residual_l0"): (690.258176e6 + 137.026304e6, "profiles/r01e_ncu_full_cfg5.md"),
 }
 LEVEL0_CLASSES = ("visit_l0", "relax_l0", "relax_l0_first", "relax_l0_last", "residual_l0")
 
