@@ -373,14 +373,14 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
             tmu, tmf, faces<T>(L0), g, fused_restrict ? s->L[1].g : g, make_coef<T>(s, 0), write_r ? (T*)L0.gsrc : nullptr,
             fused_restrict ? (T*)s->L[1].gsrc : nullptr, s->partial, mc);
         R.check(TAG_RESIDUAL0);
-        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
+        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 3.0 : 0.0));
         if (fused_restrict) R.acct(1, 1.0);
     } else {
         dim3 g = grd(L0.g);
         if (!R.plan) klaunch(R, k_residual<T, ND, VAR>, g, blk(), 0, L0.g, make_coef<T>(s, 0), (const T*)(R.u_override ? R.u_override : s->u), (const T*)s->f,
                                                        faces<T>(L0), write_r ? (T*)L0.gsrc : nullptr, s->partial);
         R.check(TAG_RESIDUAL0);
-        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 1.0 : 0.0));
+        R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 3.0 : 0.0));
         n = int(g.x * g.y * g.z);
     }
     if (!R.plan) klaunch(R, k_norm_finish, 1, 256, 0, s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
@@ -682,7 +682,7 @@ void rec_cycle(Rec& R) {
                 if (!R.plan) launch_relax_first<T, ND, VAR>(R, t, fuse_ec, (const T*)L[t + 1].a, rotp<T>(Lt, out), addu ? (T*)s->u : nullptr);
                 R.check(tag);
                 R.acct(t + 1, 2.0, tag);
-                R.acct(t, 2.0 + (VAR ? 1.0 : 0.0) + (addu ? 1.0 : 0.0), tag);
+                R.acct(t, 2.0 + (VAR ? 3.0 : 0.0) + (addu ? 1.0 : 0.0), tag);
                 prev2 = prev_in; prev_in = in; in = out;
                 continue;
             }
@@ -701,7 +701,7 @@ void rec_cycle(Rec& R) {
                                              have_d0 ? (const T*)Lt.d0 : nullptr, rotp<T>(Lt, v0), addu ? (T*)s->u : nullptr);
                 R.check(tag);
             }
-            R.acct(t, 3.0 + (VAR ? 1.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
+            R.acct(t, 3.0 + (VAR ? 3.0 : 0.0) + (book ? (a_zero[t] ? 1.0 : 2.0) + (have_d0 ? 1.0 : 0.0) + (eta > 1 ? 1.0 : 0.0) : 0.0) +
                           (addu ? (tiled(s, t) && t == 0 ? 1.0 : 2.0) : 0.0), tag);
             prev2 = prev_in; prev_in = in; in = out;
         }
@@ -746,7 +746,7 @@ T* v_sweeps(Rec& R, int m, T* cur, int n, T* final_dst) {
         } else {
             launch_relax<T, ND, VAR>(R, m, cur, out, nullptr, 0, nullptr, nullptr, nullptr);
             R.check(m == 0 ? TAG_RELAX0 : TAG_RELAX);
-            R.acct(m, 3.0 + (VAR ? 1.0 : 0.0), m == 0 ? TAG_RELAX0 : TAG_RELAX);
+            R.acct(m, 3.0 + (VAR ? 3.0 : 0.0), m == 0 ? TAG_RELAX0 : TAG_RELAX);
         }
         cur = out;
         done += ns;
@@ -786,7 +786,7 @@ void rec_vcycle(Rec& R) {
             klaunch(R, k_residual<T, ND, VAR>, grd(Lm.g), blk(), 0, Lm.g, make_coef<T>(s, m), (const T*)cur[m],
                     (const T*)Lm.gsrc, faces<T>(Lm), (T*)Lm.tmp, s->partial);
             R.check(TAG_OTHER);
-            R.acct(m, 3.0 + (VAR ? 1.0 : 0.0), TAG_OTHER);
+            R.acct(m, 3.0 + (VAR ? 3.0 : 0.0), TAG_OTHER);
             klaunch(R, k_restrict<T, ND>, grd(L[m + 1].g), blk(), 0, L[m + 1].g, Lm.g, (const T*)Lm.tmp, (T*)L[m + 1].gsrc);
             R.check(TAG_RESTRICT);
             R.acct(m, 1.0, TAG_RESTRICT); R.acct(m + 1, 1.0, TAG_RESTRICT);
