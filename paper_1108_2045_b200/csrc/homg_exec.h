@@ -10,7 +10,7 @@ enum {
     TAG_INJECT, TAG_D0, TAG_COARSE, TAG_OTHER, TAG_RELAX0_FIRST, TAG_RELAX0_LAST, TAG_VISIT0, TAG_VISIT, TAG_COUNT
 };
 
-constexpr long long kTiledMinNodesDefault = 200000;   // 65^3 and up, 449^2 and up
+constexpr long long kTiledMinNodesDefault = 300000;   // 129^3 and up, 1025^2 and up (65^3 and 513^2 measured faster on the generic kernels)
 
 // Device queries, the driver's tensor-map encoder, kernel attributes.  Called once by homg_create.
 cudaError_t exec_init(homg_solver* s);

@@ -251,9 +251,10 @@ def test_kvisit_matches_per_sweep_kernels_bitwise(orc, monkeypatch, name, n, max
     import dataclasses
     cfg = dataclasses.replace(I.scaled(I.CONFIGS[name], n), max_iters=maxi)
     inp = I.make_inputs(cfg)
-    a, na, _ = run_gpu(cfg, inp, 2)
+    # (tiled_min_nodes: 65^3 and 513^2 sit below the default threshold of the tiled kernels)
+    a, na, _ = run_gpu(cfg, inp, 2, tiled_min_nodes=200000)
     monkeypatch.setenv("HOMG_FUSE_VISIT", "0")
-    b, nb, _ = run_gpu(cfg, inp, 2)
+    b, nb, _ = run_gpu(cfg, inp, 2, tiled_min_nodes=200000)
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
     assert np.array_equal(na, nb)
@@ -262,7 +263,7 @@ def test_kvisit_matches_per_sweep_kernels_bitwise(orc, monkeypatch, name, n, max
 def test_variable_coefficient_fused_first_sweep(orc, monkeypatch):
     """k_relax_first for the variable-coefficient stencil (off by default: slower than deliver + sweep on cfg5)."""
     monkeypatch.setenv("HOMG_FUSE_FIRST_VAR", "1")
-    check_parity(I.scaled(I.CONFIGS["cfg5"], 65), 3, orc)
+    check_parity(I.scaled(I.CONFIGS["cfg5"], 65), 3, orc, tiled_min_nodes=200000)
     check_parity(I.scaled(I.CONFIGS["cfg5"], 33), 3, orc, tiled_min_nodes=1, march_chunk=6)
 
 
