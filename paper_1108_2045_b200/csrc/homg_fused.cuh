@@ -171,6 +171,15 @@ k_relax_tma(const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUt
         const Pack<T> fzp = nfz, fym = nfym, fyp = nfyp, fxp = nfx;
         const T fxl = nfxl;
         if (kok) fetch_faces(c + mstride);
+        // operands of the NEXT plane's epilogues (S4: u; S3e: v0, d0, a) into L1 now (no registers)
+        if (row_ok) {
+            if (u) asm volatile("prefetch.global.L1 [%0];" ::"l"(u + c + mstride));
+            if (a) {
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(v0 + c + mstride));
+                if (d0) asm volatile("prefetch.global.L1 [%0];" ::"l"(d0 + c + mstride));
+                if (!a_assign) asm volatile("prefetch.global.L1 [%0];" ::"l"(a + c + mstride));
+            }
+        }
         mbar_wait(&bars[sn], ((i + 1) / TL::NST) & 1);
         nxt = *reinterpret_cast<const Pack<T>*>(vs(sn) + voff);
         const T* vt = vs(sc);
