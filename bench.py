@@ -165,7 +165,7 @@ NCU_TRAFFIC = {
     ("cfg3", "visit_l0"): (693.390848e6 + 235.526656e6, "profiles/r01e_ncu_full_cfg3.md"),
     ("cfg3", "residual_l0"): (548.102656e6 + 302.414592e6, "profiles/r01e_ncu_full_cfg3.md"),
     ("cfg5", "relax_l0"): (687.057920e6 + 121.797120e6, "profiles/r01e_ncu_full_cfg5.md"),
-    ("cfg5", "relax_l0_last"): (820.713472e6 + 122.384128e6, "profiles/r01e_ncu_full_cfg5.md"),
+    ("cfg5", "relax_l0_last"): (821.715712e6 + 122.345984e6, "profiles/r01e_ncu_full_cfg5.md"),
     ("cfg5", "residual_l0"): (690.258176e6 + 137.026304e6, "profiles/r01e_ncu_full_cfg5.md"),
 }
 LEVEL0_CLASSES = ("visit_l0", "relax_l0", "relax_l0_first", "relax_l0_last", "residual_l0")
