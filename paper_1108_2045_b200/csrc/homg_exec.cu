@@ -100,7 +100,6 @@ void klaunch(Rec& R, K kern, dim3 grid, dim3 block, size_t smem, Args... args) {
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
     if (R.err == cudaSuccess && e != cudaSuccess) R.err = e;
 }
-inline dim3 d3(int x) { return dim3(x, 1, 1); }
 
 // resident CTAs per SM of a kernel at its launch configuration (asked of the runtime once per kernel): the
 // marching-axis chunk counts are chosen so that tiles x chunks fills whole waves of sm_count x this
