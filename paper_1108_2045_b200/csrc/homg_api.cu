@@ -1,5 +1,6 @@
 // homg_api.cu — the C ABI of libhomg.so (include/homg.h): argument checking, workspace carving,
 // graph capture and replay.  No arithmetic of the method happens on the host.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>

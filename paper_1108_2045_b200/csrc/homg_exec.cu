@@ -360,9 +360,23 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         long long tiles = (long long)((g.nx - 1 + TL::TX - 1) / TL::TX) * (ND == 3 ? (g.ny - 1 + TL::TY - 1) / TL::TY : 1);
         int mc = s->march_chunk;
         if (mc <= 0) {
+            // chunk count: fill whole waves of (148 x resident CTAs) as evenly as possible — an SM with fewer CTAs than
+            // its residency cannot draw its share of the bandwidth — at little halo overhead (2 planes per chunk)
             const int occ = resident_ctas(k_res_tma<T, ND, VAR>, TL::NW * 32, res_smem_bytes<T, ND, VAR>());
-            long long nch = std::max<long long>(1, (long long)s->sm_count * occ / std::max<long long>(tiles, 1));
-            mc = std::max(int((interior + nch - 1) / nch), 8);
+            const long long slots = (long long)s->sm_count * occ;
+            // (one wave that fills >= 80 % of the slots is kept: measured best on cfg3 / cfg5; cfg4's 256 tiles fill 58 %)
+            double best = -1.0, best1 = -1.0;
+            int bestn = 1, bestn1 = 1;
+            for (int nch = 1; nch <= std::max(1, interior / 8); ++nch) {
+                const int m = (interior + nch - 1) / nch;
+                const long long ctas = tiles * nch, waves = (ctas + slots - 1) / slots;
+                const double score = double(ctas) / double(waves * slots) * double(m) / double(m + 2);
+                if (score > best + 1e-9) { best = score; bestn = nch; }
+                if (waves == 1 && score > best1 + 1e-9) { best1 = score; bestn1 = nch; }
+                if (waves > 8) break;
+            }
+            if (best1 >= 0.8) bestn = bestn1;
+            mc = (interior + bestn - 1) / bestn;
         }
         mc = (mc + 1) & ~1;                                        // even: chunks start on odd planes
         int nch = (interior + mc - 1) / mc;
