@@ -157,8 +157,8 @@ def find_cstar(s, d, cfg):
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from `ncu --set full`
 # captures, one launch each; the summaries and their commands are under profiles/.
 NCU_TRAFFIC = {
-    ("cfg4", "visit_l0"): (1.318701e9 + 0.513753e9, "profiles/r01d_ncu_full_cfg4.md"),
-    ("cfg4", "residual_l0"): (1.136458e9 + 0.573487e9, "profiles/r01d_ncu_full_cfg4.md"),
+    ("cfg4", "visit_l0"): (1.318703e9 + 0.514103e9, "profiles/r01e_ncu_full_cfg4.md"),
+    ("cfg4", "residual_l0"): (1.152890e9 + 0.571569e9, "profiles/r01e_ncu_full_cfg4.md"),
     ("cfg4", "relax_l0"): (1.164186e9 + 0.509018e9, "profiles/r01b_ncu_full_cfg4.md"),
     ("cfg2", "visit_l0"): (43.483904e6 + 0.012800e6, "profiles/r01d_ncu_full_cfg2.md"),      # L2-resident (17 MB arrays)
     ("cfg2", "residual_l0"): (36.909056e6 + 0.042752e6, "profiles/r01d_ncu_full_cfg2.md"),
