@@ -10,8 +10,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "homg_oracle.cpp")
 LIB = os.path.join(HERE, "libhomg_oracle.so")
 
-# -ffp-contract=off: the oracle's arithmetic is exactly the expression tree written
-# in the source (no fused multiply-adds), so a reader can check it by eye.
+# -ffp-contract=off: the compiler contracts nothing by itself, so the oracle's arithmetic is exactly the
+# expression tree written in the source and a reader can check it by eye.  The only fused multiply-adds
+# are the three explicit std::fma calls of the constant-coefficient Jacobi sweep (Eq. 3, R14).
 CMD = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-ffp-contract=off", "-o", LIB, SRC]
 
 
