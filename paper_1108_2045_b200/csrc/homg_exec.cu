@@ -12,6 +12,7 @@
 #include "homg_coarse.cuh"
 #include "homg_first.cuh"
 #include "homg_visit.cuh"
+#include "homg_visit3.cuh"
 #include "homg_moves.cuh"
 #include "homg_literal.cuh"
 
@@ -293,9 +294,60 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
                 make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
 }
 
+// K_visit, 3-D form (homg_visit3.cuh): two rows per thread, g carried in registers
+template <class T, int NS, bool INTERP>
+void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
+                   const T* d0, const T* v0, T* u) {
+    homg_solver* s = R.s;
+    Level& Lt = s->L[t];
+    using TL = Visit3Tile<T, NS>;
+    CUtensorMap tm_in, tm_ac, tm_g;
+    bool ok = make_tmap<T, 3>(s, &tm_g, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::TXN, TL::PY);
+    if (INTERP) {
+        Level& Lc = s->L[t + 1];
+        ok = ok && make_tmap<T, 3>(s, &tm_in, ec, Lc.g, TL::CW, TL::CR) && make_tmap<T, 3>(s, &tm_ac, ac, Lc.g, TL::CW, TL::CR);
+    } else {
+        ok = ok && make_tmap<T, 3>(s, &tm_in, in, Lt.g, TL::TXN, TL::PY);
+        tm_ac = tm_in;
+    }
+    if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
+    const LevelGeom& g = Lt.g;
+    const int interior = std::max(g.nz - 2, 1);
+    const int tx = (g.nx - 1 + TL::OX - 1) / TL::OX, ty = (g.ny - 1 + TL::OY - 1) / TL::OY;
+    const long long tiles = (long long)tx * ty;
+    const long long slots = s->sm_count;                           // one CTA per SM
+    // z chunks (even length): the count that minimises waves x (planes per chunk + pipeline fill and drain)
+    int best = 1;
+    double bestc = 1e300;
+    for (int nch = 1; nch <= 256 && nch <= std::max(1, interior / 2); ++nch) {
+        const int mc = ((interior + nch - 1) / nch + 1) & ~1;
+        const int n = (interior + mc - 1) / mc;
+        const long long waves = (tiles * n + slots - 1) / slots;
+        const double c = double(waves) * double(mc + 2 * NS + 8);
+        if (c < bestc) { bestc = c; best = nch; }
+    }
+    int mc = s->march_chunk > 0 ? std::min(s->march_chunk, interior) : (interior + best - 1) / best;
+    mc = (mc + 1) & ~1;
+    const int nch = (interior + mc - 1) / mc;
+    dim3 grid(tx, ty, nch);
+    const bool bookv = !INTERP && (a || o1 || o2);
+    if (bookv)
+        klaunch(R, k_visit3<T, NS, false, true>, grid, TL::NT, visit3_smem_bytes<T, NS, false>(), tm_in, tm_ac, tm_g, g,
+                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+    else
+        klaunch(R, k_visit3<T, NS, INTERP, false>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
+                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+}
+
 template <class T, int ND, bool INTERP>
 void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
                      int a_assign, const T* d0, const T* v0, T* u) {
+    if (ND == 3 && R.s->visit3) {
+        if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+        else if (ns == 3) launch_visit3<T, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+        else launch_visit3<T, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+        return;
+    }
     if (ns == 2) launch_visit<T, ND, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
     else if (ns == 3) launch_visit<T, ND, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
     else launch_visit<T, ND, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
@@ -952,7 +1004,13 @@ cudaError_t set_attr_visit1() {
 template <class T, int NS>
 cudaError_t set_attr_visit() {
     cudaError_t e = set_attr_visit1<T, 2, NS>();
-    return e != cudaSuccess ? e : set_attr_visit1<T, 3, NS>();
+    if (e != cudaSuccess) return e;
+    if ((e = set_attr_visit1<T, 3, NS>()) != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_visit3<T, NS, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_visit3<T, NS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_visit3<T, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, true>());
 }
 
 }  // namespace
