@@ -66,6 +66,7 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
 // q mod UNR of a step: a compile-time constant in the steady loop, q itself elsewhere
 template <int N>
@@ -250,27 +251,45 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         const int KV = K & (TL::NIN - 1), KP = (K + TL::NIN - 1) & (TL::NIN - 1);   // ring slots of planes q, q-1
         const int z0 = zs + q;
         const bool zodd = (1 + NS + K) & 1;                        // parity of z0 (ms is odd)
-        // ---- stage 0: the packs of v^0 at plane z0 ----
+        // ---- stage 0: the packs of v^0 at plane z0 (registers only, so far) ----
         Pack<T> nx[2];
         if (INTERP) {
             produce(z0, zodd, nx);
-            *reinterpret_cast<Pack<T>*>(buf(0, W) + offE) = nx[0];
-            *reinterpret_cast<Pack<T>*>(buf(0, W) + offO) = nx[1];
         } else {
             mbar_wait(&fbar[KV], (q / TL::NIN) & 1);
             nx[0] = *reinterpret_cast<const Pack<T>*>(vring(KV) + offE);
             nx[1] = *reinterpret_cast<const Pack<T>*>(vring(KV) + offO);
         }
+        // ---- every thread has finished the shared-memory traffic of step q-1 (it arrived after its last stage
+        // store; its last stage, its epilogue and the stage 0 above hide the skew between warps) ----
+        if (STEADY || q >= 1) {
+            mbar_wait(&sbar, R);
+            if (tid == 0) {                                        // ring slots of planes q-1 are free: refill
+                const int i = q + TL::NIN - 2;
+                if (!INTERP && i < nsteps) issue_v(i);
+                if (i <= nsteps - 2) issue_g(i);
+                if (INTERP && !zodd) {                             // plane z0-1 was odd: coarse plane (z0-1)>>1 is dead
+                    const int zc = ((z0 - 1) >> 1) - Zc0 + TL::NC;
+                    if (zc < ncz) issue_c(zc);
+                }
+            }
+        }
+        if (INTERP) {
+            *reinterpret_cast<Pack<T>*>(buf(0, W) + offE) = nx[0];
+            *reinterpret_cast<Pack<T>*>(buf(0, W) + offO) = nx[1];
+        }
         const bool fin = STEADY || q >= 2 * NS;
-        // operands of this step's epilogue: global -> shared now (cp.async, no registers: with ~200 KB of shared
-        // memory there is no L1 left to prefetch into), read after the NS stages
-        if (fin) {
+        // operands of the epilogues: global -> shared by cp.async (no registers; with ~200 KB of shared memory
+        // there is no L1 left to prefetch into).  Level 0 (u streams from DRAM): issued one step ahead into the
+        // other slot; levels >= 1 (v^0, d0, a: L2-resident): issued now for this step.  One group per step.
+        {
+            const bool pre = !BOOK && (STEADY || (q + 1 >= 2 * NS && q + 1 < nsteps));
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 if (!own[r]) continue;
                 const long long c = cF + r * rowO;
-                if (!BOOK && u) cp_async16(eps(0, r), u + c);
-                if (BOOK && a) {
+                if (pre && u) cp_async16(eps(R, r), u + c + mstride);
+                if (BOOK && fin && a) {
                     cp_async16(eps(0, r), v0 + c);
                     if (d0) cp_async16(eps(1, r), d0 + c);
                     if (!a_assign) cp_async16(eps(2, r), a + c);
@@ -334,7 +353,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             // all shared-memory traffic of this step that other threads see is done (stage NS's neighbours were
             // fetched above): arrive now, wait at the end of the step — the last stage and the epilogue hide the skew
             if (s == NS - 1) mbar_arrive(&sbar);
-            if (s == NS && fin) cp_async_wait_all();
+            if (s == NS && fin) { if (BOOK) cp_async_wait_all(); else cp_async_wait_1(); }
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 if (!own[r]) continue;
@@ -357,7 +376,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                         *reinterpret_cast<Pack<T>*>(a + c) = aa;
                     }
                     if (!BOOK && u) {                              // S4: u += v^NS
-                        Pack<T> uu = *reinterpret_cast<const Pack<T>*>(eps(0, r));
+                        Pack<T> uu = *reinterpret_cast<const Pack<T>*>(eps(W, r));
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) uu.v[j] += out[r].v[j];
                         *reinterpret_cast<Pack<T>*>(u + c) = uu;
@@ -370,16 +389,6 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
 #pragma unroll
         for (int s = NS - 2; s >= 1; --s) { Gh[s][0] = Gh[s - 1][0]; Gh[s][1] = Gh[s - 1][1]; }
         Gh[0][0] = gn[0]; Gh[0][1] = gn[1];
-        mbar_wait(&sbar, W);
-        if (tid == 0) {
-            const int i = q + TL::NIN - 1;
-            if (!INTERP && i < nsteps) issue_v(i);
-            if (i <= nsteps - 2) issue_g(i);
-            if (INTERP && zodd) {                                  // coarse plane z0>>1 is dead now
-                const int zc = (z0 >> 1) - Zc0 + TL::NC;
-                if (zc < ncz) issue_c(zc);
-            }
-        }
         cF += mstride;
     };
     int q = 0;
