@@ -149,7 +149,7 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST")) s->fuse_first = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST_VAR")) s->fuse_first_var = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
-    if (const char* ev = std::getenv("HOMG_VISIT3")) s->visit3 = std::atoi(ev) != 0;
+    if (const char* ev = std::getenv("HOMG_VISIT3")) s->visit3 = std::atoi(ev);
     s->vcycle = o.cycle == HOMG_CYCLE_V;
     s->literal = o.cycle == HOMG_CYCLE_LITERAL;
     s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;

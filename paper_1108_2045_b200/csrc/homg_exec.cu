@@ -295,12 +295,12 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
 }
 
 // K_visit, 3-D form (homg_visit3.cuh): two rows per thread, g carried in registers
-template <class T, int NS, bool INTERP>
-void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
-                   const T* d0, const T* v0, T* u) {
+template <class T, int NS, bool INTERP, bool BOOK>
+void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
+                    const T* d0, const T* v0, T* u) {
     homg_solver* s = R.s;
     Level& Lt = s->L[t];
-    using TL = Visit3Tile<T, NS>;
+    using TL = Visit3Tile<T, NS, BOOK>;
     CUtensorMap tm_in, tm_ac, tm_g;
     bool ok = make_tmap<T, 3>(s, &tm_g, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::TXN, TL::PY);
     if (INTERP) {
@@ -330,19 +330,22 @@ void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, 
     mc = (mc + 1) & ~1;
     const int nch = (interior + mc - 1) / mc;
     dim3 grid(tx, ty, nch);
-    const bool bookv = !INTERP && (a || o1 || o2);
-    if (bookv)
-        klaunch(R, k_visit3<T, NS, false, true>, grid, TL::NT, visit3_smem_bytes<T, NS, false>(), tm_in, tm_ac, tm_g, g,
-                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
-    else
-        klaunch(R, k_visit3<T, NS, INTERP, false>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP>(), tm_in, tm_ac, tm_g, g,
-                make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+    klaunch(R, k_visit3<T, NS, INTERP, BOOK>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP, BOOK>(), tm_in, tm_ac, tm_g, g,
+            make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+}
+template <class T, int NS, bool INTERP>
+void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
+                   const T* d0, const T* v0, T* u) {
+    if (!INTERP && (a || o1 || o2)) launch_visit3b<T, NS, false, true>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+    else launch_visit3b<T, NS, INTERP, false>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
 }
 
 template <class T, int ND, bool INTERP>
 void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
                      int a_assign, const T* d0, const T* v0, T* u) {
-    if (ND == 3 && R.s->visit3) {
+    // (the S3e-bookkeeping form of levels >= 1 stays on homg_visit.cuh unless visit3 == 2: k_visit3<.., BOOK> needs
+    // more registers than 384 threads leave it)
+    if (ND == 3 && R.s->visit3 && (R.s->visit3 >= 2 || INTERP || !(a || o1 || o2))) {
         if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
         else if (ns == 3) launch_visit3<T, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
         else launch_visit3<T, 4, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
@@ -1006,11 +1009,11 @@ cudaError_t set_attr_visit() {
     cudaError_t e = set_attr_visit1<T, 2, NS>();
     if (e != cudaSuccess) return e;
     if ((e = set_attr_visit1<T, 3, NS>()) != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_visit3<T, NS, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false>());
+    e = cudaFuncSetAttribute(k_visit3<T, NS, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false, false>());
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_visit3<T, NS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false>());
+    e = cudaFuncSetAttribute(k_visit3<T, NS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false, true>());
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_visit3<T, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, true>());
+    return cudaFuncSetAttribute(k_visit3<T, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, true, false>());
 }
 
 }  // namespace

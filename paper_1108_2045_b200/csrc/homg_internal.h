@@ -83,7 +83,7 @@ struct homg_solver {
     bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
     int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
-    bool visit3 = true;              // 3-D K_visit: homg_visit3.cuh (HOMG_VISIT3=0: the r01 kernel of homg_visit.cuh)
+    int visit3 = 1;                  // 3-D K_visit: homg_visit3.cuh (HOMG_VISIT3=0: the r01 kernel of homg_visit.cuh)
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create
     std::vector<int> sched_lv, sched_it;

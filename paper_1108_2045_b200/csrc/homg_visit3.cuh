@@ -23,11 +23,13 @@
 
 namespace homg {
 
-template <class T, int NS>
+// BOOK: the visit of a level >= 1 (S3e bookkeeping, three iterates stored) carries more live values per thread:
+// 320 threads (20 row pairs) at <= 204 registers instead of 384 at <= 168
+template <class T, int NS, bool BOOK>
 struct Visit3Tile {
     static constexpr int ES = int(sizeof(T));
     static constexpr int VEC = 16 / ES;
-    static constexpr int PX = 16, TR = 24, NT = PX * TR;       // packs per row, row pairs, threads
+    static constexpr int PX = 16, TR = BOOK ? 20 : 24, NT = PX * TR;   // packs per row, row pairs, threads
     static constexpr int HX = (NS + VEC - 1) / VEC * VEC;      // x halo (nodes), pack granular
     static constexpr int HY = (NS + 1) / 2 * 2;                // y halo (rows), row-pair granular
     static constexpr int TXN = PX * VEC, PY = 2 * TR;          // tile in nodes
@@ -47,17 +49,18 @@ struct Visit3Tile {
     // epilogue operands (u; or v^0, d0, a) of a step: one 16-byte slot per thread and row, filled by cp.async at the
     // start of the step and read after the NS stages (up to 3 arrays)
     static constexpr int EP_BYTES = 2 * NT * 16;
+    static constexpr int NEP = BOOK ? 6 : 2;                   // slots: level 0: u of this / the next step; BOOK: 3 arrays x 2
     static_assert(CW >= CWN + VEC - 1, "coarse tile too narrow");
     static_assert(PLANE_BYTES % 128 == 0 && BOX_BYTES % 128 == 0, "TMA destinations are 128-B aligned");
     static_assert(NIN == UNR && NG == UNR && NC == UNR, "ring slots are compile-time constants of the unrolled loop");
 };
 
-template <class T, int NS, bool INTERP>
+template <class T, int NS, bool INTERP, bool BOOK>
 __host__ __device__ constexpr int visit3_smem_bytes() {
-    using TL = Visit3Tile<T, NS>;
+    using TL = Visit3Tile<T, NS, BOOK>;
     return TL::NG * TL::BOX_BYTES +
            (INTERP ? TL::NC * 2 * TL::CTILE_BYTES + NS * 2 * TL::PLANE_BYTES
-                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + 3 * TL::EP_BYTES + 128;
+                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + TL::NEP * TL::EP_BYTES + 128;
 }
 
 // cp.async (LDGSTS): 16 bytes global -> shared without passing through registers; completion per thread
@@ -76,14 +79,14 @@ __device__ __forceinline__ int step_k(int q) { return q; }
 // Arguments as k_visit (homg_visit.cuh).  grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior
 // planes); mchunk must be even when there is more than one chunk (every chunk then starts on an odd plane).
 template <class T, int NS, bool INTERP, bool BOOK>
-__global__ void __launch_bounds__(Visit3Tile<T, NS>::NT, 1)
+__global__ void __launch_bounds__(Visit3Tile<T, NS, BOOK>::NT, 1)
 k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
          const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
          T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
          const T* __restrict__ v0, T* __restrict__ u, int mchunk) {
     pdl_start();
     static_assert(!(INTERP && BOOK), "interpolate+correct is fused on level 0 only");
-    using TL = Visit3Tile<T, NS>;
+    using TL = Visit3Tile<T, NS, BOOK>;
     constexpr int VEC = TL::VEC, RS = TL::RS;
     const int tid = threadIdx.x, px = tid % TL::PX, tr = tid / TL::PX;
     const int NM = g.nz;
@@ -279,20 +282,20 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             *reinterpret_cast<Pack<T>*>(buf(0, W) + offO) = nx[1];
         }
         const bool fin = STEADY || q >= 2 * NS;
-        // operands of the epilogues: global -> shared by cp.async (no registers; with ~200 KB of shared memory
-        // there is no L1 left to prefetch into).  Level 0 (u streams from DRAM): issued one step ahead into the
-        // other slot; levels >= 1 (v^0, d0, a: L2-resident): issued now for this step.  One group per step.
+        // operands of the NEXT step's epilogue (u; or v^0, d0, a): global -> shared by cp.async, one step ahead into
+        // the other slot (no registers; with ~200 KB of shared memory there is no L1 left to prefetch into).
+        // One group per step.
         {
-            const bool pre = !BOOK && (STEADY || (q + 1 >= 2 * NS && q + 1 < nsteps));
+            const bool pre = STEADY || (q + 1 >= 2 * NS && q + 1 < nsteps);
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
-                if (!own[r]) continue;
-                const long long c = cF + r * rowO;
-                if (pre && u) cp_async16(eps(R, r), u + c + mstride);
-                if (BOOK && fin && a) {
-                    cp_async16(eps(0, r), v0 + c);
-                    if (d0) cp_async16(eps(1, r), d0 + c);
-                    if (!a_assign) cp_async16(eps(2, r), a + c);
+                if (!own[r] || !pre) continue;
+                const long long c = cF + r * rowO + mstride;
+                if (!BOOK && u) cp_async16(eps(R, r), u + c);
+                if (BOOK && a) {
+                    cp_async16(eps(R, r), v0 + c);
+                    if (d0) cp_async16(eps(2 + R, r), d0 + c);
+                    if (!a_assign) cp_async16(eps(4 + R, r), a + c);
                 }
             }
             cp_async_commit();
@@ -353,7 +356,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             // all shared-memory traffic of this step that other threads see is done (stage NS's neighbours were
             // fetched above): arrive now, wait at the end of the step — the last stage and the epilogue hide the skew
             if (s == NS - 1) mbar_arrive(&sbar);
-            if (s == NS && fin) { if (BOOK) cp_async_wait_all(); else cp_async_wait_1(); }
+            if (s == NS && fin) cp_async_wait_1();
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 if (!own[r]) continue;
@@ -365,9 +368,9 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 if (s == NS && fin) {
                     if (o0) *reinterpret_cast<Pack<T>*>(o0 + c) = out[r];
                     if (BOOK && a) {                               // S3e: a (+)= d0 + v^{NS-1} - v^0
-                        Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(eps(0, r)), aa;
-                        if (d0) dd = *reinterpret_cast<const Pack<T>*>(eps(1, r));
-                        if (!a_assign) aa = *reinterpret_cast<const Pack<T>*>(eps(2, r));
+                        Pack<T> dd, vv = *reinterpret_cast<const Pack<T>*>(eps(W, r)), aa;
+                        if (d0) dd = *reinterpret_cast<const Pack<T>*>(eps(2 + W, r));
+                        if (!a_assign) aa = *reinterpret_cast<const Pack<T>*>(eps(4 + W, r));
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) {
                             const T Dq = ((d0 ? dd.v[j] : T(0)) + C[s - 1][r].v[j]) - vv.v[j];
