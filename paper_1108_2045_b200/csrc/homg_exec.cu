@@ -301,7 +301,7 @@ void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0,
     homg_solver* s = R.s;
     Level& Lt = s->L[t];
     using TL = Visit3Tile<T, NS, BOOK>;
-    CUtensorMap tm_in, tm_ac, tm_g;
+    CUtensorMap tm_in, tm_ac, tm_g, tm_u;
     bool ok = make_tmap<T, 3>(s, &tm_g, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::TXN, TL::PY);
     if (INTERP) {
         Level& Lc = s->L[t + 1];
@@ -310,6 +310,8 @@ void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0,
         ok = ok && make_tmap<T, 3>(s, &tm_in, in, Lt.g, TL::TXN, TL::PY);
         tm_ac = tm_in;
     }
+    if (u && !BOOK) ok = ok && make_tmap<T, 3>(s, &tm_u, u, Lt.g, TL::OX, TL::OY);
+    else tm_u = tm_g;
     if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
     const LevelGeom& g = Lt.g;
     const int interior = std::max(g.nz - 2, 1);
@@ -330,7 +332,7 @@ void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0,
     mc = (mc + 1) & ~1;
     const int nch = (interior + mc - 1) / mc;
     dim3 grid(tx, ty, nch);
-    klaunch(R, k_visit3<T, NS, INTERP, BOOK>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP, BOOK>(), tm_in, tm_ac, tm_g, g,
+    klaunch(R, k_visit3<T, NS, INTERP, BOOK>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP, BOOK>(), tm_in, tm_ac, tm_g, tm_u, g,
             make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
 }
 template <class T, int NS, bool INTERP>

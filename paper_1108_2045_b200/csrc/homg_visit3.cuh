@@ -49,7 +49,11 @@ struct Visit3Tile {
     // epilogue operands (u; or v^0, d0, a) of a step: one 16-byte slot per thread and row, filled by cp.async at the
     // start of the step and read after the NS stages (up to 3 arrays)
     static constexpr int EP_BYTES = 2 * NT * 16;
-    static constexpr int NEP = BOOK ? 6 : 2;                   // slots: level 0: u of this / the next step; BOOK: 3 arrays x 2
+    static constexpr int NEP = BOOK ? 6 : 0;                   // BOOK: 3 arrays x 2 slots
+    // level 0: the stored region of u, one TMA box {OX, OY, 1} per step, NU slots (issued two steps ahead)
+    static constexpr int NU = 4;
+    static constexpr int UBOX_BYTES = OX * OY * ES;
+    static_assert(UBOX_BYTES % 128 == 0 && (OX * ES) % 16 == 0, "u box: 128-B aligned slots, 16-B rows");
     static_assert(CW >= CWN + VEC - 1, "coarse tile too narrow");
     static_assert(PLANE_BYTES % 128 == 0 && BOX_BYTES % 128 == 0, "TMA destinations are 128-B aligned");
     static_assert(NIN == UNR && NG == UNR && NC == UNR, "ring slots are compile-time constants of the unrolled loop");
@@ -60,7 +64,7 @@ __host__ __device__ constexpr int visit3_smem_bytes() {
     using TL = Visit3Tile<T, NS, BOOK>;
     return TL::NG * TL::BOX_BYTES +
            (INTERP ? TL::NC * 2 * TL::CTILE_BYTES + NS * 2 * TL::PLANE_BYTES
-                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + TL::NEP * TL::EP_BYTES + 128;
+                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + TL::NEP * TL::EP_BYTES + (BOOK ? 0 : TL::NU * TL::UBOX_BYTES) + 128;
 }
 
 // cp.async (LDGSTS): 16 bytes global -> shared without passing through registers; completion per thread
@@ -70,6 +74,56 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+
+// ---- one Jacobi stage on a pack: out = v + w_p ((sum_nb v - 2d v) + h^2 g), Eq. 3 in the order of DESIGN.md R14 ----
+// generic (fp64): one scalar operation per node and term
+template <class T>
+__device__ __forceinline__ Pack<T> jacobi_pack(const Pack<T>& pv, const Pack<T>& cu, const Pack<T>& nx, const Pack<T>& dn,
+                                               const Pack<T>& up, const Pack<T>& gv, T vl, T vr, const Pack<T>& wpm,
+                                               const Coef<T>& cf) {
+    constexpr int VEC = 16 / int(sizeof(T));
+    Pack<T> out;
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+        const T vc = cu.v[j];
+        const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
+        const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+        T sm = pv.v[j] + nx.v[j];
+        sm += dn.v[j] + up.v[j];
+        sm += xm + xp;
+        T t = fma_rn(-cf.twod, vc, sm);
+        t = fma_rn(cf.h2, gv.v[j], t);
+        out.v[j] = fma_rn(wpm.v[j], t, vc);
+    }
+    return out;
+}
+// fp32: sm_100a packed pairs (add / fma .rn.f32x2 = FADD2 / FFMA2: two IEEE round-to-nearest operations per
+// instruction, so the results are those of the scalar form bit for bit).  A pack is two pairs (v0,v1), (v2,v3) —
+// the register pairs LDS.128 / STS.128 already use; only the x-neighbour sums (vl+v1, v0+v2), (v1+v3, v2+vr) pair
+// nodes differently and are formed by four scalar additions.  18 instructions per pack instead of 32.
+struct F2 { unsigned long long b; };
+__device__ __forceinline__ F2 f2_make(float lo, float hi) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.b) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void f2_get(F2 a, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.b)); }
+__device__ __forceinline__ F2 f2_add(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.b) : "l"(a.b), "l"(b.b)); return r; }
+__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.b) : "l"(a.b), "l"(b.b), "l"(c.b)); return r; }
+__device__ __forceinline__ Pack<float> jacobi_pack(const Pack<float>& pv, const Pack<float>& cu, const Pack<float>& nx,
+                                                   const Pack<float>& dn, const Pack<float>& up, const Pack<float>& gv,
+                                                   float vl, float vr, const Pack<float>& wpm, const Coef<float>& cf) {
+    const F2 ntd = f2_make(-cf.twod, -cf.twod), h2 = f2_make(cf.h2, cf.h2);
+    const float xs[4] = {vl + cu.v[1], cu.v[0] + cu.v[2], cu.v[1] + cu.v[3], cu.v[2] + vr};
+    Pack<float> out;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const F2 c2 = f2_make(cu.v[2 * h], cu.v[2 * h + 1]);
+        F2 sm = f2_add(f2_make(pv.v[2 * h], pv.v[2 * h + 1]), f2_make(nx.v[2 * h], nx.v[2 * h + 1]));
+        sm = f2_add(sm, f2_add(f2_make(dn.v[2 * h], dn.v[2 * h + 1]), f2_make(up.v[2 * h], up.v[2 * h + 1])));
+        sm = f2_add(sm, f2_make(xs[2 * h], xs[2 * h + 1]));
+        F2 t = f2_fma(ntd, c2, sm);
+        t = f2_fma(h2, f2_make(gv.v[2 * h], gv.v[2 * h + 1]), t);
+        f2_get(f2_fma(f2_make(wpm.v[2 * h], wpm.v[2 * h + 1]), t, c2), out.v[2 * h], out.v[2 * h + 1]);
+    }
+    return out;
+}
 
 // q mod UNR of a step: a compile-time constant in the steady loop, q itself elsewhere
 template <int N>
@@ -81,7 +135,7 @@ __device__ __forceinline__ int step_k(int q) { return q; }
 template <class T, int NS, bool INTERP, bool BOOK>
 __global__ void __launch_bounds__(Visit3Tile<T, NS, BOOK>::NT, 1)
 k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
-         const __grid_constant__ CUtensorMap tm_g, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
+         const __grid_constant__ CUtensorMap tm_g, const __grid_constant__ CUtensorMap tm_u, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
          T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
          const T* __restrict__ v0, T* __restrict__ u, int mchunk) {
     pdl_start();
@@ -102,7 +156,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
 
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-    __shared__ uint64_t fbar[TL::NIN], gbar[TL::NG], cbar[TL::NC], sbar;
+    __shared__ uint64_t fbar[TL::NIN], gbar[TL::NG], cbar[TL::NC], ubar[TL::NU], sbar;
     auto gs = [&](int st) { return reinterpret_cast<T*>(smem + st * TL::BOX_BYTES); };
     unsigned char* cbase = smem + TL::NG * TL::BOX_BYTES;          // PLAIN: v ring;  INTERP: coarse ring
     auto vring = [&](int st) { return reinterpret_cast<T*>(cbase + st * TL::PLANE_BYTES); };
@@ -112,6 +166,8 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
     constexpr int NBUF = INTERP ? NS : NS - 1;
     unsigned char* epbase = sbase + NBUF * 2 * TL::PLANE_BYTES;
     auto eps = [&](int arr, int r) { return reinterpret_cast<T*>(epbase + arr * TL::EP_BYTES + (r * TL::NT + tid) * 16); };
+    auto us = [&](int st) { return reinterpret_cast<T*>(epbase + TL::NEP * TL::EP_BYTES + st * TL::UBOX_BYTES); };
+    const bool stage_u = !BOOK && u != nullptr;
     auto buf = [&](int s, int slot) {                              // plane published by stage s
         return reinterpret_cast<T*>(sbase + ((INTERP ? s : s - 1) * 2 + slot) * TL::PLANE_BYTES);
     };
@@ -121,6 +177,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         for (int s = 0; s < TL::NG; ++s) mbar_init(&gbar[s], 1);
         for (int s = 0; s < TL::NC; ++s) mbar_init(&cbar[s], 1);
         mbar_init(&sbar, TL::NT);
+        for (int s = 0; s < TL::NU; ++s) mbar_init(&ubar[s], 1);
         mbar_fence_init();
     }
     // the pad rows of every plane are read as the y neighbours of the first / last tile row (halo rows whose
@@ -149,6 +206,11 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         mbar_arrive_expect_tx(&gbar[st], TL::BOX_BYTES);
         tma_load_3d(gs(st), &tm_g, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
     };
+    auto issue_u = [&](int i) {                                    // stored region of u at the plane step i finishes
+        const int st = i & (TL::NU - 1);
+        mbar_arrive_expect_tx(&ubar[st], TL::UBOX_BYTES);
+        tma_load_3d(us(st), &tm_u, &ubar[st], x0, y0, zs + i - NS);
+    };
     auto issue_c = [&](int zc) {                                   // coarse plane Zc0+zc of e_c and a_c
         const int st = zc & (TL::NC - 1);
         mbar_arrive_expect_tx(&cbar[st], 2 * TL::CBOX_BYTES);
@@ -161,6 +223,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
         for (int i = 0; i < TL::NIN - 1 && i < nsteps; ++i) {
             if (!INTERP) issue_v(i);
             if (i <= nsteps - 2) issue_g(i);
+            if (stage_u) issue_u(i);
         }
     }
 
@@ -170,17 +233,18 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
     const int offE = TL::ROFF + (2 * tr) * RS + px * VEC, offO = offE + RS;   // in a padded plane
     const int goffE = (2 * tr) * RS + px * VEC, goffO = goffE + RS;
     // Eq. 3 multiplier w_p of every node; 0 where the node is not an interior node of the level
-    T wpm[2][VEC];
+    Pack<T> wpm[2];
     bool own[2];
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
         const int y = ye + r;
         const bool row_int = y > 0 && y < g.ny - 1;
 #pragma unroll
-        for (int j = 0; j < VEC; ++j) wpm[r][j] = (row_int && x + j > 0 && x + j < g.nx - 1) ? cf.wp : T(0);
+        for (int j = 0; j < VEC; ++j) wpm[r].v[j] = (row_int && x + j > 0 && x + j < g.nx - 1) ? cf.wp : T(0);
         own[r] = px * VEC >= TL::HX && px * VEC < TL::HX + TL::OX && x < g.nx && 2 * tr + r >= TL::HY &&
                  2 * tr + r < TL::HY + TL::OY && y < g.ny;
     }
+    const int uoff = (2 * tr - TL::HY) * TL::OX + px * VEC - TL::HX;   // my even row in a u box (own threads only)
     const int coff = tr * TL::CW + (Xc - Xa) + px * (VEC / 2);     // INTERP: my first coarse node, coarse row ye/2
 
     // S3a in registers: the two packs of v^0 at fine plane z (rows ye even, ye+1 odd) from the coarse planes
@@ -271,6 +335,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 const int i = q + TL::NIN - 2;
                 if (!INTERP && i < nsteps) issue_v(i);
                 if (i <= nsteps - 2) issue_g(i);
+                if (stage_u && q + 2 < nsteps) issue_u(q + 2);     // (its slot was last read in step q-2)
                 if (INTERP && !zodd) {                             // plane z0-1 was odd: coarse plane (z0-1)>>1 is dead
                     const int zc = ((z0 - 1) >> 1) - Zc0 + TL::NC;
                     if (zc < ncz) issue_c(zc);
@@ -291,14 +356,13 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             for (int r = 0; r < 2; ++r) {
                 if (!own[r] || !pre) continue;
                 const long long c = cF + r * rowO + mstride;
-                if (!BOOK && u) cp_async16(eps(R, r), u + c);
                 if (BOOK && a) {
                     cp_async16(eps(R, r), v0 + c);
                     if (d0) cp_async16(eps(2 + R, r), d0 + c);
                     if (!a_assign) cp_async16(eps(4 + R, r), a + c);
                 }
             }
-            cp_async_commit();
+            if (BOOK) cp_async_commit();
         }
         // g of plane z0-1: from its ring into registers, once; stage s reads it s-1 steps from now
         Pack<T> gn[2];
@@ -336,17 +400,10 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 const Pack<T>& gv = s == 1 ? gn[r] : Gh[s == 1 ? 0 : s - 2][r];
                 const T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
                 const T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
+                out[r] = jacobi_pack(pv, cu, nx[r], dn, up, gv, vl, vr, wpm[r], cf);
+                if (!zin) {                                        // Dirichlet planes z = 0, nz-1 (and beyond)
 #pragma unroll
-                for (int j = 0; j < VEC; ++j) {
-                    const T vc = cu.v[j];
-                    const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
-                    const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-                    T sm = pv.v[j] + nx[r].v[j];
-                    sm += dn.v[j] + up.v[j];
-                    sm += xm + xp;
-                    T t = fma_rn(-cf.twod, vc, sm);                // Eq. 3 (jacobi_eq3 with the per-node w_p)
-                    t = fma_rn(cf.h2, gv.v[j], t);
-                    out[r].v[j] = zin ? fma_rn(wpm[r][j], t, vc) : T(0);
+                    for (int j = 0; j < VEC; ++j) out[r].v[j] = T(0);
                 }
             }
             if (s < NS) {
@@ -356,7 +413,10 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             // all shared-memory traffic of this step that other threads see is done (stage NS's neighbours were
             // fetched above): arrive now, wait at the end of the step — the last stage and the epilogue hide the skew
             if (s == NS - 1) mbar_arrive(&sbar);
-            if (s == NS && fin) cp_async_wait_1();
+            if (s == NS) {                                         // (every issued u box is waited for: none in flight at exit)
+                if (BOOK && fin) cp_async_wait_1();
+                if (!BOOK && stage_u) mbar_wait(&ubar[K & (TL::NU - 1)], (q / TL::NU) & 1);
+            }
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 if (!own[r]) continue;
@@ -379,7 +439,7 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                         *reinterpret_cast<Pack<T>*>(a + c) = aa;
                     }
                     if (!BOOK && u) {                              // S4: u += v^NS
-                        Pack<T> uu = *reinterpret_cast<const Pack<T>*>(eps(W, r));
+                        Pack<T> uu = *reinterpret_cast<const Pack<T>*>(us(K & (TL::NU - 1)) + uoff + r * TL::OX);
 #pragma unroll
                         for (int j = 0; j < VEC; ++j) uu.v[j] += out[r].v[j];
                         *reinterpret_cast<Pack<T>*>(u + c) = uu;
