@@ -146,6 +146,18 @@ HOMG_API homg_status homg_set_coefficient(homg_solver* s, const void* k, int on_
  * fp64, no h^d factor — DESIGN.md R12). */
 HOMG_API homg_status homg_cycle(homg_solver* s, int n);
 
+/* Cycles until the residual is small: runs outer cycles (as homg_cycle) until
+ * || f - A u ||_2 <= rel_tol * || f - A u_0 ||_2  (u_0 = the initial guess: the first history entry) or
+ * max_cycles cycles have run — PAPER.md L75: "the residual equation is used to restart the cycles as many
+ * times as needed to reach any desired accuracy".  The loop runs ON THE DEVICE: one CUDA graph whose WHILE node
+ * repeats the cycle body, the residual-norm kernel at the end of every cycle setting the loop condition; the host
+ * is not involved between the launch and the end of the solve (no transfer, no synchronisation inside).  The call
+ * then synchronises the stream and reads back the cycle count and two norms (20 bytes).  History: one entry per
+ * cycle run (the norm before it), as homg_cycle.  *cycles_done = cycles run by this call, *rel_residual = final
+ * || r || / || r_0 || (either may be NULL).  HOMG_CYCLE_MFMG only (not mixed precision): HOMG_ESTATE otherwise.
+ * HOMG_EINVAL if history_cap < cycles already run + max_cycles + 1. */
+HOMG_API homg_status homg_solve(homg_solver* s, double rel_tol, int max_cycles, int* cycles_done, double* rel_residual);
+
 /* || f - A u ||_2 of the CURRENT u (one norm-only pass, stream sync, 8-byte D2H) and its
  * ratio to the first history entry (the norm of the initial guess; 1 if no cycle ran).
  * Either output pointer may be NULL. */

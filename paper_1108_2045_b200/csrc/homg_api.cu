@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "homg_exec.h"
 
@@ -37,6 +38,51 @@ homg_status cuda_fail(homg_solver* s, cudaError_t e, const char* where) {
 void drop_graph(homg_solver* s) {
     if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
     if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+    if (s->solve_exec) { cudaGraphExecDestroy(s->solve_exec); s->solve_exec = nullptr; }
+    if (s->solve_graph) { cudaGraphDestroy(s->solve_graph); s->solve_graph = nullptr; }
+}
+
+struct SolveParamsHost { double tol2; int max_slot; int pad; };   // = SolveParams of homg_kernels.cuh
+
+// homg_solve's graph: [S1 of the initial guess] -> WHILE (norm above tolerance) { S2..S4 of one cycle; S1 of the new u }.
+// Both parts are captured from the executor's launch sequence; the norm kernel sets the condition on the device.
+homg_status build_solve_graph(homg_solver* s) {
+    CU(s, cudaGraphCreate(&s->solve_graph, 0));
+    cudaGraphConditionalHandle h;
+    cudaError_t e = cudaGraphConditionalHandleCreate(&h, s->solve_graph, 1, cudaGraphCondAssignDefault);
+    if (e == cudaSuccess) e = cudaStreamBeginCaptureToGraph(s->cap_stream, s->solve_graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: graph prologue"); }
+    e = exec_solve_prologue(s, s->cap_stream, (unsigned long long)h);
+    cudaGraph_t got = nullptr;
+    cudaError_t e2 = cudaStreamEndCapture(s->cap_stream, &got);
+    if (e != cudaSuccess || e2 != cudaSuccess) { drop_graph(s); return cuda_fail(s, e != cudaSuccess ? e : e2, "homg_solve: capture(prologue)"); }
+    // the WHILE node depends on the leaves of the prologue
+    size_t nn = 0, ne = 0;
+    CU(s, cudaGraphGetNodes(s->solve_graph, nullptr, &nn));
+    std::vector<cudaGraphNode_t> nodes(nn);
+    CU(s, cudaGraphGetNodes(s->solve_graph, nodes.data(), &nn));
+    CU(s, cudaGraphGetEdges(s->solve_graph, nullptr, nullptr, &ne));
+    std::vector<cudaGraphNode_t> from(ne), to(ne);
+    if (ne) CU(s, cudaGraphGetEdges(s->solve_graph, from.data(), to.data(), &ne));
+    std::vector<cudaGraphNode_t> leaves;
+    for (auto n : nodes) if (std::find(from.begin(), from.end(), n) == from.end()) leaves.push_back(n);
+    cudaGraphNodeParams p = {};
+    p.type = cudaGraphNodeTypeConditional;
+    p.conditional.handle = h;
+    p.conditional.type = cudaGraphCondTypeWhile;
+    p.conditional.size = 1;
+    cudaGraphNode_t cn;
+    e = cudaGraphAddNode(&cn, s->solve_graph, leaves.data(), leaves.size(), &p);
+    if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: conditional node"); }
+    cudaGraph_t body = p.conditional.phGraph_out[0];
+    e = cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: graph body"); }
+    e = exec_solve_body(s, s->cap_stream, (unsigned long long)h);
+    e2 = cudaStreamEndCapture(s->cap_stream, &got);
+    if (e != cudaSuccess || e2 != cudaSuccess) { drop_graph(s); return cuda_fail(s, e != cudaSuccess ? e : e2, "homg_solve: capture(body)"); }
+    e = cudaGraphInstantiate(&s->solve_exec, s->solve_graph, 0);
+    if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: cudaGraphInstantiate"); }
+    return HOMG_OK;
 }
 
 homg_status reset_history(homg_solver* s) {
@@ -194,6 +240,7 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     s->hist = static_cast<double*>(take(size_t(hist_cap) * sizeof(double)));
     s->slot = static_cast<int*>(take(256));
     s->scalar = reinterpret_cast<double*>(reinterpret_cast<char*>(s->slot) + 128);
+    s->solve_params = reinterpret_cast<char*>(s->slot) + 64;
     if (size_t(p - s->ws_base) > ws_bytes) { delete s; return set_err(nullptr, HOMG_ENOMEM, "internal: layout exceeds plan"); }
 
     cudaError_t e = cudaMemsetAsync(ws, 0, size_t(p - s->ws_base), s->stream);
@@ -265,6 +312,41 @@ homg_status homg_cycle(homg_solver* s, int n) {
         else CU(s, exec_cycle(s, s->stream));
     }
     s->cycles_issued += n;
+    return HOMG_OK;
+}
+
+homg_status homg_solve(homg_solver* s, double rel_tol, int max_cycles, int* cycles_done, double* rel_residual) {
+    if (!s) return HOMG_EINVAL;
+    if (!(rel_tol >= 0) || max_cycles < 0) return set_err(s, HOMG_EINVAL, "homg_solve: rel_tol >= 0 and max_cycles >= 0");
+    if (!s->have_rhs) return set_err(s, HOMG_ESTATE, "homg_solve before homg_set_rhs");
+    if (s->var && !s->have_coef) return set_err(s, HOMG_ESTATE, "homg_solve before homg_set_coefficient");
+    if (s->inner || s->vcycle || s->literal)
+        return set_err(s, HOMG_ESTATE, "homg_solve runs the MFMG cycle (HOMG_CYCLE_MFMG, not mixed precision); use homg_cycle");
+    const long start = s->cycles_issued;
+    if (start + max_cycles + 1 > s->hist_cap) return set_err(s, HOMG_EINVAL, "homg_solve: history_cap too small for max_cycles");
+    CU(s, exec_prepare(s));
+    if (!s->solve_exec) {
+        homg_status r = build_solve_graph(s);
+        if (r != HOMG_OK) return r;
+    }
+    SolveParamsHost sp{rel_tol * rel_tol, int(start + max_cycles), 0};
+    CU(s, cudaMemcpyAsync(s->solve_params, &sp, sizeof(sp), cudaMemcpyHostToDevice, s->stream));
+    CU(s, cudaGraphLaunch(s->solve_exec, s->stream));
+    // the solve is over when the stream is: read back how far it went (one int, two doubles)
+    int slot = 0;
+    CU(s, cudaMemcpyAsync(&slot, s->slot, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    if (slot < start + 1) return set_err(s, HOMG_ECUDA, "homg_solve: the device loop did not run");
+    double n2[2] = {0, 0};
+    CU(s, cudaMemcpyAsync(&n2[0], s->hist, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaMemcpyAsync(&n2[1], s->hist + (slot - 1), sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    // the last entry is the norm of the final u = the norm BEFORE the next cycle: the next cycle records it again
+    const int keep = slot - 1;
+    CU(s, cudaMemcpyAsync(s->slot, &keep, sizeof(int), cudaMemcpyHostToDevice, s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    s->cycles_issued = keep;
+    if (cycles_done) *cycles_done = int(keep - start);
+    if (rel_residual) *rel_residual = n2[0] > 0 ? std::sqrt(n2[1] / n2[0]) : 0.0;
     return HOMG_OK;
 }
 

@@ -8,6 +8,7 @@
 #include <cstdlib>
 
 #include <cstring>
+#include <mutex>
 
 #include "homg_coarse.cuh"
 #include "homg_first.cuh"
@@ -37,6 +38,14 @@ struct Rec {                 // bookkeeping while recording
     const void* g_override = nullptr;         // V-cycle, level 0: the sweeps' right-hand side is f, not g_0
     const void* u_override = nullptr;         // V-cycle: the residual is taken of this iterate instead of u
     bool plan = false;                        // planning pass: build the coarse program, launch nothing
+    // homg_solve (a CUDA-graph WHILE node loops the cycle on the device): S1 runs at the END of the body on the new
+    // u, and its norm kernel sets the loop condition.  Inside a conditional body the first and the last kernel are
+    // launched without the programmatic (PDL) attribute (measured: a PDL-attributed last kernel lets the next
+    // iteration start early and loses updates).
+    bool s1_at_end = false;
+    unsigned long long cond = 0;              // cudaGraphConditionalHandle; 0: plain cycle
+    bool nopdl_next = false;                  // the next launch carries no PDL attribute
+    bool pdl_now() { const bool p = s->pdl && !nopdl_next; nopdl_next = false; return p; }
     std::vector<unsigned char> prog;          // CoarseOp records of the whole cycle, in order
     int prog_nops = 0, run_begin = 0, run_len = 0;
     long long run_maxnodes = 0;
@@ -50,6 +59,7 @@ struct Rec {                 // bookkeeping while recording
         ++prog_nops; ++run_len;
         if (nodes > run_maxnodes) run_maxnodes = nodes;
     }
+    void note(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; }
     void acct(int level, double arrays, int tag) { last_tag = tag; acct(level, arrays); }
     // a fused multi-sweep launch: `arrays` = the per-sweep (algorithmic) passes it stands for,
     // `comp` = the passes the fused launch itself has to move
@@ -63,7 +73,8 @@ struct Rec {                 // bookkeeping while recording
         if (plan) return;
         cudaError_t e = cudaPeekAtLastError();
         static const bool dbg = std::getenv("HOMG_DEBUG_SYNC") != nullptr;   // localise a faulting launch
-        if (dbg && e == cudaSuccess) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (dbg && e == cudaSuccess && cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusNone) {
             e = cudaStreamSynchronize(st);
             if (e != cudaSuccess) std::fprintf(stderr, "homg: launch %d (tag %d) failed: %s\n", launches, tag, cudaGetErrorString(e));
         }
@@ -96,7 +107,7 @@ void klaunch(Rec& R, K kern, dim3 grid, dim3 block, size_t smem, Args... args) {
     cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = R.st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = R.s->pdl ? 1 : 0;
+    at[0].val.programmaticStreamSerializationAllowed = R.pdl_now() ? 1 : 0;
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
     if (R.err == cudaSuccess && e != cudaSuccess) R.err = e;
@@ -106,8 +117,12 @@ void klaunch(Rec& R, K kern, dim3 grid, dim3 block, size_t smem, Args... args) {
 // marching-axis chunk counts are chosen so that tiles x chunks fills whole waves of sm_count x this
 template <class K>
 int resident_ctas(K kern, int threads, size_t smem) {
-    static std::vector<std::pair<const void*, int>> cache;       // keyed by the kernel's address (one K per signature)
+    // keyed by the kernel's address (one K per signature, one launch configuration per kernel); solvers may be
+    // created and cycled from several threads
+    static std::mutex mu;
+    static std::vector<std::pair<const void*, int>> cache;
     const void* key = reinterpret_cast<const void*>(kern);
+    std::lock_guard<std::mutex> lock(mu);
     for (auto& c : cache) if (c.first == key) return c.second;
     int n = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, smem) != cudaSuccess || n < 1) n = 1;
@@ -385,7 +400,7 @@ void flush_run(Rec& R) {
             at[0].id = cudaLaunchAttributeClusterDimension;
             at[0].val.clusterDim.x = ncta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
             at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            at[1].val.programmaticStreamSerializationAllowed = s->pdl ? 1 : 0;
+            at[1].val.programmaticStreamSerializationAllowed = R.pdl_now() ? 1 : 0;
             cfg.attrs = at; cfg.numAttrs = 2;
             cudaError_t e = ncta > 1 ? cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, true>, dev, n)
                                      : cudaLaunchKernelEx(&cfg, k_coarse_run<T, ND, VAR, false>, dev, n);
@@ -453,8 +468,16 @@ bool rec_norm(Rec& R, bool write_r, bool to_history, bool restrict1 = false) {
         R.acct(0, (write_r ? 3.0 : 2.0) + (VAR ? 3.0 : 0.0));
         n = int(g.x * g.y * g.z);
     }
-    if (!R.plan) klaunch(R, k_norm_finish, 1, 256, 0, s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
-                                        to_history ? 1 : 0, to_history ? nullptr : s->scalar);
+    if (!R.plan) {
+        if (R.cond) {                                            // homg_solve: the norm decides whether the loop goes on
+            R.nopdl_next = true;
+            klaunch(R, k_norm_finish_solve, 1, 256, 0, s->partial, n, s->hist, s->slot, s->hist_cap, (const SolveParams*)s->solve_params,
+                    R.cond);
+        } else {
+            klaunch(R, k_norm_finish, 1, 256, 0, s->partial, n, to_history ? s->hist : nullptr, s->slot, s->hist_cap,
+                    to_history ? 1 : 0, to_history ? nullptr : s->scalar);
+        }
+    }
     R.check(TAG_NORM_FINISH);
     return fused_restrict;
 }
@@ -477,7 +500,9 @@ void rec_cycle(Rec& R) {
     auto flush = [&]() { flush_run<T, ND, VAR>(R); };
 
     // S1: r = f - A u, ||r||^2 -> history
-    const bool have_g1 = R.skip_s1 ? false : rec_norm<T, ND, VAR>(R, true, true, true);
+    // (homg_solve: S1 of this cycle ran at the end of the previous loop body, or in the prologue)
+    if (R.s1_at_end) R.nopdl_next = true;
+    const bool have_g1 = R.skip_s1 ? false : R.s1_at_end ? (tiled(s, 0) && s->levels >= 2) : rec_norm<T, ND, VAR>(R, true, true, true);
     // S2: nested restriction g_m = P g_{m-1}
     for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
         if (small(m)) {
@@ -500,6 +525,13 @@ void rec_cycle(Rec& R) {
         bool have_d0 = false;
         bool fuse_first = false;
         const T* fuse_ec = nullptr;
+        // K_visit runs this visit (decided here because a level-0 visit in MID-cycle must leave v^{eta-1} behind for
+        // the carried variation of the next visit: K_visit stores it only in its bookkeeping form, which takes its
+        // v^0 from memory — such a visit is not fused with its arrival)
+        const int kv_maxns = std::min(s->fuse_visit, 4);
+        const bool use_kvisit = !VAR && kv_maxns >= 2 && tiled(s, t) && !(s->coarse_threshold > 0 && Lt.n_nodes <= s->coarse_threshold) &&
+                                eta >= 2 && (t == 0 || eta <= kv_maxns);
+        const bool mid_l0 = t == 0 && vi != nv - 1;
         if (cur < 0) {
             if (small(t)) {
                 CoarseOp<T> o = newop(OP_ZERO, t);
@@ -507,7 +539,7 @@ void rec_cycle(Rec& R) {
                 R.push(o, L[t].n_nodes);
             } else {
                 flush();
-                if (!R.plan) cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st);
+                if (!R.plan) R.note(cudaMemsetAsync(Lt.rot[Lt.e], 0, Lt.n_alloc * sizeof(T), R.st));
                 R.check(TAG_OTHER);
             }
             Lt.touched = true;
@@ -525,7 +557,8 @@ void rec_cycle(Rec& R) {
                     Level& Lc = L[m];
                     Level& Lf = L[m - 1];
                     int ef_assign = Lf.touched ? 0 : 1;
-                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && (VAR ? s->fuse_first_var : s->fuse_first)) {
+                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && (VAR ? s->fuse_first_var : s->fuse_first) &&
+                        !(use_kvisit && mid_l0)) {
                         fuse_first = true;                   // S3a of this hop happens inside the first sweep
                         fuse_ec = rotp<T>(Lc, Lc.e);
                         Lf.touched = true;
@@ -638,14 +671,14 @@ void rec_cycle(Rec& R) {
                 R.push(o, Lt.n_nodes);
             } else {
                 flush();
-                if (!R.plan) cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st);
+                if (!R.plan) R.note(cudaMemsetAsync(Lt.d0, 0, Lt.n_alloc * sizeof(T), R.st));
                 R.check(TAG_OTHER);
             }
             have_d0 = true;
         }
         // K_visit: the whole visit (or, on level 0, chunks of up to 4 sweeps) in one pass over HBM
-        const int maxns = std::min(s->fuse_visit, 4);
-        if (!VAR && maxns >= 2 && tiled(s, t) && !small(t) && eta >= 2 && (t == 0 || eta <= maxns)) {
+        const int maxns = kv_maxns;
+        if (use_kvisit) {
             flush();
             const int v0i = Lt.e;
             int in = v0i, i1 = -1, i2 = -1, done = 0;           // rot indices of v^k, v^{k-1}, v^{k-2}
@@ -668,7 +701,7 @@ void rec_cycle(Rec& R) {
                 int ob[3] = {-1, -1, -1}, nb = 0;               // free buffers: not the input, not v^0 (t >= 1)
                 for (int b = 0; b < Lt.nrot && nb < 3; ++b)
                     if (b != in && !(t >= 1 && b == v0i)) ob[nb++] = b;
-                const int b0 = ob[0], b1 = t >= 1 ? ob[1] : -1, b2 = (t >= 1 && ns >= 3) ? ob[2] : -1;
+                const int b0 = ob[0], b1 = (t >= 1 || (mid_l0 && lastc)) ? ob[1] : -1, b2 = (t >= 1 && ns >= 3) ? ob[2] : -1;
                 T* o0 = addu ? nullptr : rotp<T>(Lt, b0);
                 const int tag = t == 0 ? TAG_VISIT0 : TAG_VISIT;
                 if (!R.plan) {
@@ -781,6 +814,7 @@ void rec_cycle(Rec& R) {
         cur = t;
     }
     flush();
+    if (R.s1_at_end) rec_norm<T, ND, VAR>(R, true, true, true);    // S1 + S5 of the new u: the loop condition
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -837,7 +871,7 @@ void rec_vcycle(Rec& R) {
         Level& Lm = L[m];
         if (m >= 1) {                                            // e_m = 0
             cur[m] = rotp<T>(Lm, 0);
-            cudaMemsetAsync(cur[m], 0, Lm.n_alloc * sizeof(T), R.st);
+            R.note(cudaMemsetAsync(cur[m], 0, Lm.n_alloc * sizeof(T), R.st));
             R.check(TAG_OTHER);
         }
         R.g_override = m == 0 ? s->f : nullptr;
@@ -865,7 +899,7 @@ void rec_vcycle(Rec& R) {
     // (c) coarsest level: exact solve (one interior node)
     cur[M] = rotp<T>(L[M], 0);
     if (M >= 1) {
-        cudaMemsetAsync(cur[M], 0, L[M].n_alloc * sizeof(T), R.st);
+        R.note(cudaMemsetAsync(cur[M], 0, L[M].n_alloc * sizeof(T), R.st));
         R.check(TAG_OTHER);
         klaunch(R, k_coarsest_solve<T, ND, VAR>, dim3(1), dim3(32), 0, L[M].g, make_coef<T>(s, M), (const T*)L[M].gsrc,
                 faces<T>(L[M]), cur[M]);
@@ -881,7 +915,7 @@ void rec_vcycle(Rec& R) {
         R.g_override = nullptr;
     }
     if (cur[0] != (T*)s->u) {                                    // eta2 = 0, or a single sweep that started from u
-        cudaMemcpyAsync(s->u, cur[0], L[0].n_alloc * sizeof(T), cudaMemcpyDeviceToDevice, R.st);
+        R.note(cudaMemcpyAsync(s->u, cur[0], L[0].n_alloc * sizeof(T), cudaMemcpyDeviceToDevice, R.st));
         R.check(TAG_OTHER);
         R.acct(0, 2.0, TAG_OTHER);
     }
@@ -904,8 +938,8 @@ void rec_literal(Rec& R) {
         R.acct(m - 1, 1.0, TAG_RESTRICT); R.acct(m, 1.0, TAG_RESTRICT);
     }
     int ic = 0, ip = 1, in = 2;                                                // cur, prev, nxt among the 3 level-0 buffers
-    cudaMemsetAsync(L0.rot[ic], 0, L0.n_alloc * sizeof(T), R.st); R.check(TAG_OTHER);
-    cudaMemsetAsync(L0.rot[ip], 0, L0.n_alloc * sizeof(T), R.st); R.check(TAG_OTHER);
+    R.note(cudaMemsetAsync(L0.rot[ic], 0, L0.n_alloc * sizeof(T), R.st)); R.check(TAG_OTHER);
+    R.note(cudaMemsetAsync(L0.rot[ip], 0, L0.n_alloc * sizeof(T), R.st)); R.check(TAG_OTHER);
     R.acct(0, 2.0, TAG_OTHER);
     for (size_t vi = 0; vi < s->sched_lv.size(); ++vi) {
         const int m = s->sched_lv[vi];
@@ -1062,9 +1096,9 @@ cudaError_t exec_prepare(homg_solver* s) {
     if (P.err != cudaSuccess) return P.err;
     if (!P.prog.empty()) {
         cudaError_t e = cudaMalloc(&s->prog_dev, P.prog.size());
-        if (e != cudaSuccess) return e;
+        if (e != cudaSuccess) { s->prog_dev = nullptr; return e; }
         e = cudaMemcpy(s->prog_dev, P.prog.data(), P.prog.size(), cudaMemcpyHostToDevice);
-        if (e != cudaSuccess) return e;
+        if (e != cudaSuccess) { cudaFree(s->prog_dev); s->prog_dev = nullptr; return e; }
     }
     s->prog_ready = true;
     return cudaSuccess;
@@ -1086,7 +1120,7 @@ cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st) {
     klaunch(R, k_cvt4<ND, false>, g4, blk(), 0, go, gi, (double*)s->L[0].gsrc, (float*)in->L[0].gsrc);
     R.check(TAG_OTHER);
     R.acct(0, 1.5, TAG_OTHER);
-    cudaMemsetAsync(in->u, 0, in->L[0].n_alloc * sizeof(float), st);
+    R.note(cudaMemsetAsync(in->u, 0, in->L[0].n_alloc * sizeof(float), st));
     R.check(TAG_OTHER);
     R.acct(0, 0.5, TAG_OTHER);
     Rec Ri{in, st};
@@ -1117,6 +1151,26 @@ cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
     if (s->vcycle) HOMG_DISPATCH(s, rec_vcycle, R);
     else if (s->literal) HOMG_DISPATCH(s, rec_literal, R);
     else HOMG_DISPATCH(s, rec_cycle, R);
+    s->launches_per_cycle = R.launches;
+    s->bytes_cycle_all = R.bytes_all;
+    s->bytes_cycle_l0 = R.bytes_l0;
+    for (int t = 0; t < TAG_COUNT; ++t) s->comp_by_tag[t] = R.comp_tag[t];
+    return R.err;
+}
+
+// homg_solve, prologue: S1 of the initial guess (norm -> history, loop condition)
+cudaError_t exec_solve_prologue(homg_solver* s, cudaStream_t st, unsigned long long cond) {
+    Rec R{s, st};
+    R.cond = cond;
+    HOMG_DISPATCH(s, rec_norm, R, true, true, true);
+    return R.err;
+}
+// homg_solve, loop body: S2..S4 of one cycle, then S1 of the new u
+cudaError_t exec_solve_body(homg_solver* s, cudaStream_t st, unsigned long long cond) {
+    Rec R{s, st};
+    R.cond = cond;
+    R.s1_at_end = true;
+    HOMG_DISPATCH(s, rec_cycle, R);
     s->launches_per_cycle = R.launches;
     s->bytes_cycle_all = R.bytes_all;
     s->bytes_cycle_l0 = R.bytes_l0;

@@ -26,6 +26,10 @@ cudaError_t exec_prepare(homg_solver* s);
 // Issues the launches of ONE outer cycle on `st` (which may be a capturing stream) and fills
 // s->launches_per_cycle / s->bytes_cycle_*.
 cudaError_t exec_cycle(homg_solver* s, cudaStream_t st);
+// homg_solve: the launches of the prologue (S1 of the initial guess) and of the loop body (S2..S4, then S1 of the
+// new u) of the device-side WHILE loop; `cond` is the cudaGraphConditionalHandle the norm kernel sets.
+cudaError_t exec_solve_prologue(homg_solver* s, cudaStream_t st, unsigned long long cond);
+cudaError_t exec_solve_body(homg_solver* s, cudaStream_t st, unsigned long long cond);
 // One cycle with plain stream launches, an event after every launch; accumulates the elapsed ms and
 // launch counts per TAG_* (arrays of TAG_COUNT).  Synchronises the stream.
 cudaError_t exec_cycle_profiled(homg_solver* s, cudaStream_t st, double* ms_by_tag, int* launches_by_tag,

@@ -104,6 +104,9 @@ struct homg_solver {
     cudaStream_t cap_stream = nullptr;   // private stream used only to capture the graph
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
+    cudaGraph_t solve_graph = nullptr;   // homg_solve: S1, then a WHILE node whose body is one cycle (S2..S4, S1)
+    cudaGraphExec_t solve_exec = nullptr;
+    void* solve_params = nullptr;        // device: SolveParams (tolerance^2, last history slot)
     bool have_rhs = false, have_coef = false;
     long cycles_issued = 0;
     int launches_per_cycle = 0;

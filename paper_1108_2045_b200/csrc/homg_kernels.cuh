@@ -173,6 +173,30 @@ __global__ void k_norm_finish(const double* __restrict__ partial, int n, double*
     }
 }
 
+// homg_solve: the same sum; the new norm^2 goes to hist[*slot] and decides whether the device-side loop (a CUDA
+// graph WHILE node) runs another cycle: while ||r_c||^2 > tol^2 ||r_0||^2 and c < max_cycles   (PAPER.md L75:
+// "restart the cycles as many times as needed to reach any desired accuracy")
+struct SolveParams {
+    double tol2;        // (relative tolerance)^2
+    int max_slot;       // history index at which the loop stops regardless (cycles already issued + max_cycles)
+};
+__global__ void k_norm_finish_solve(const double* __restrict__ partial, int n, double* __restrict__ hist,
+                                    int* __restrict__ slot, int cap, const SolveParams* __restrict__ sp,
+                                    unsigned long long cond) {
+    pdl_start();
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) s += partial[i];
+    double t = block_sum(s);
+    if (threadIdx.x == 0) {
+        const int c = *slot;
+        if (c < cap) hist[c] = t;
+        *slot = c + 1;
+        const double first = c == 0 ? t : hist[0];
+        const bool go = c < sp->max_slot && c + 1 < cap && t > sp->tol2 * first;
+        cudaGraphSetConditional(cudaGraphConditionalHandle(cond), go ? 1u : 0u);
+    }
+}
+
 // full weighting: coarse interior node I = sum_{delta in {-1,0,1}^d} 2^(-d-|delta|_1) fine(2I+delta);
 // coarse boundary entries 0.  Grid over the COARSE level.
 template <class T, int ND>

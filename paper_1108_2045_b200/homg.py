@@ -19,7 +19,7 @@ DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
 # every symbol include/homg.h declares (tests check that the library exports each one)
 SYMBOLS = [
     "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
-    "homg_set_coefficient", "homg_cycle", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
+    "homg_set_coefficient", "homg_cycle", "homg_solve", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
     "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_workspace_bytes_mixed", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
 ]
 
@@ -61,6 +61,7 @@ def lib():
         for name in ("homg_set_rhs", "homg_set_initial_guess", "homg_set_coefficient", "homg_get_solution"):
             getattr(L, name).argtypes = [vp, vp, i]; getattr(L, name).restype = i
         L.homg_cycle.argtypes = [vp, i]; L.homg_cycle.restype = i
+        L.homg_solve.argtypes = [vp, d, i, C.POINTER(i), C.POINTER(d)]; L.homg_solve.restype = i
         L.homg_residual_norm.argtypes = [vp, C.POINTER(d), C.POINTER(d)]; L.homg_residual_norm.restype = i
         L.homg_residual_history.argtypes = [vp, C.POINTER(d), i, C.POINTER(i)]; L.homg_residual_history.restype = i
         L.homg_get_schedule.argtypes = [vp, C.POINTER(i), C.POINTER(i), i]; L.homg_get_schedule.restype = i
@@ -172,6 +173,13 @@ class Solver:
     def cycle(self, n=1):
         with self._torch.cuda.device(self.device):
             self._ck(lib().homg_cycle(self.handle, int(n)))
+
+    def solve(self, rel_tol, max_cycles):
+        """homg_solve: cycles on the device until ||r|| <= rel_tol ||r_0|| or max_cycles; (cycles run, final ||r||/||r_0||)."""
+        n = C.c_int(0); r = C.c_double(0)
+        with self._torch.cuda.device(self.device):
+            self._ck(lib().homg_solve(self.handle, float(rel_tol), int(max_cycles), C.byref(n), C.byref(r)))
+        return n.value, r.value
 
     def residual_norm(self):
         a = C.c_double(0); r = C.c_double(0)

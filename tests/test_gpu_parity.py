@@ -65,7 +65,7 @@ def check_parity(cfg, ncycles, orc, floor=None, **kw):
         if onorms[c] / onorms[0] < floor:
             break
         fg, fo = norms[c] / norms[c - 1], onorms[c] / onorms[c - 1]
-        assert abs(fg - fo) <= 5e-3 * abs(fo) * (1 if cfg.dtype == "f32" else 0.2), (cfg.name, c, fg, fo)
+        assert abs(fg - fo) <= 5e-4 * abs(fo), (cfg.name, c, fg, fo)       # 3 significant digits (north_star)
     return us, norms
 
 
@@ -123,6 +123,23 @@ def test_explicit_schedule_with_single_iterations_and_fine_revisits(orc):
     cfg3 = I.scaled(I.CONFIGS["cfg2"], 17)
     sched3 = ([3, 1, 0, 2, 3, 0], [1, 1, 2, 1, 2, 2])
     check_parity(cfg3, 3, orc, sched=sched3)
+
+
+@pytest.mark.parametrize("fuse_first", ["1", "0"])
+def test_explicit_schedule_mid_cycle_fine_visits_on_tiled_levels(orc, monkeypatch, fuse_first):
+    """a level-0 visit of eta >= 2 in MID-cycle followed by a move up, on grids where K_visit runs level 0
+    (tiled_min_nodes=1): the carried variation of the next visit needs v^{eta-1} of that visit
+    (the r01 executor left it unset: ADVICE r1)."""
+    monkeypatch.setenv("HOMG_FUSE_FIRST", fuse_first)
+    cfg3 = I.scaled(I.CONFIGS["cfg4"], 33)
+    sched3 = ([4, 3, 2, 1, 0, 1, 0, 2, 1, 0], [2, 2, 2, 3, 4, 2, 2, 2, 4, 3])
+    check_parity(cfg3, 3, orc, sched=sched3, tiled_min_nodes=1)
+    cfg64 = I.scaled(I.CONFIGS["cfg2"], 33)
+    sched64 = ([4, 2, 0, 1, 0, 3, 0], [2, 4, 6, 2, 5, 1, 4])          # eta > 4 on level 0: chunked K_visit + a trailing sweep
+    check_parity(cfg64, 3, orc, sched=sched64, tiled_min_nodes=1)
+    cfg2d = I.scaled(I.CONFIGS["cfg3"], 257)
+    sched2d = ([7, 6, 3, 1, 0, 1, 0, 2, 0], [2, 2, 4, 4, 4, 2, 3, 2, 2])
+    check_parity(cfg2d, 3, orc, sched=sched2d, tiled_min_nodes=1)
 
 
 def test_ragged_dims_and_fewer_levels(orc):
@@ -283,7 +300,7 @@ def check_vcycle(cfg, ncycles, orc, eta=(2, 1), **kw):
         if onorms[c] / onorms[0] < floor:
             break
         fg, fo = norms[c] / norms[c - 1], onorms[c] / onorms[c - 1]
-        assert abs(fg - fo) <= 5e-3 * abs(fo), (cfg.name, c, fg, fo)
+        assert abs(fg - fo) <= 5e-4 * abs(fo), (cfg.name, c, fg, fo)
     return norms
 
 
@@ -342,20 +359,106 @@ def test_literal_and_per_level_forms_agree(orc):
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times (graph replay, default
 # ---- thresholds): the oracle runs the first cycle(s) of the same solve and EVERY node is compared ----
-@pytest.mark.parametrize("name,ncyc", [("cfg2", 4), ("cfg5", 3), ("cfg3", 2), ("cfg4", 2)])
+@pytest.mark.parametrize("name,ncyc", [("cfg2", 14), ("cfg5", 3), ("cfg3", 2), ("cfg4", 2)])
 def test_full_size_first_cycles_vs_oracle(orc, name, ncyc):
+    """cfg2: the whole solve (14 cycles to 1e-8); cfg3-5: the first cycles.  u is compared after EVERY cycle."""
     cfg = I.CONFIGS[name]
     inp = I.make_inputs(cfg)
     us, norms, sched = run_gpu(cfg, inp, ncyc)
-    u_o, _, onorms = orc.homg("H", inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, ncyc, k=inp["k"], keep_history=False)
-    ref = u_o.astype(np.float64)
-    err = np.max(np.abs(us[-1].astype(np.float64) - ref)) / np.max(np.abs(ref))
-    assert err <= TOL[cfg.dtype], f"{name} full size: {err:.3e}"
+    _, hist, onorms = orc.homg("H", inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, ncyc, k=inp["k"], keep_history=True)
+    for c in range(ncyc):
+        ref = hist[c]
+        err = float(np.max(np.abs(us[c] - ref))) / float(np.max(np.abs(ref)))
+        assert err <= TOL[cfg.dtype], f"{name} full size, cycle {c}: {err:.3e}"
     assert np.allclose(norms, onorms, rtol=1e-5 if cfg.dtype == "f32" else 1e-10)
+    if name == "cfg2":
+        assert onorms[14] <= cfg.tol * onorms[0] < onorms[13]       # 14 cycles is what 1e-8 takes
     # Dirichlet boundary stays exactly 0
     u = us[-1]
     for ax in range(u.ndim):
         assert not np.any(np.take(u, [0, -1], axis=ax))
+
+
+# ---- homg_solve: the solve stops by itself (PAPER.md L75; a device-side WHILE loop over the cycle) ----
+def oracle_cycles_to_tol(orc, cfg, inp, tol, cap):
+    sched = orc.schedule(cfg.schedule, cfg.levels, cfg.max_iters)
+    _, _, norms = orc.homg("H", inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, cap, k=inp["k"], keep_history=False)
+    for c, v in enumerate(norms):
+        if v <= tol * norms[0]:
+            return c, norms
+    return cap, norms
+
+
+@pytest.mark.parametrize("name,n,tol,kw", [("cfg2", 65, 1e-8, {}), ("cfg5", 33, 1e-8, {}), ("cfg4", 65, 1e-4, {"tiled_min_nodes": 200000}),
+                                           ("cfg3", 513, 1e-3, {"tiled_min_nodes": 200000}), ("cfg1", 129, 1e-6, {}),
+                                           ("cfg2", 33, 1e-8, {"tiled_min_nodes": 1})])
+def test_solve_stops_by_itself(orc, name, n, tol, kw):
+    _torch()
+    from paper_1108_2045_b200 import homg
+    cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+    inp = I.make_inputs(cfg)
+    cap = 40
+    want, onorms = oracle_cycles_to_tol(orc, cfg, inp, tol, cap)
+    assert 2 <= want < cap
+    def mk():
+        s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters, **kw)
+        if inp["k"] is not None:
+            s.set_coefficient(inp["k"])
+        s.set_rhs(inp["f"])
+        s.set_initial_guess(inp["u0"])
+        return s
+    s = mk()
+    done, rel = s.solve(tol, cap)
+    assert done == want, (done, want)                                   # the oracle's count
+    u = s.get_solution().copy()
+    hist = s.residual_history()
+    assert len(hist) == done
+    assert np.allclose(hist, onorms[:done], rtol=1e-5 if cfg.dtype == "f32" else 1e-10)
+    final, rel2 = s.residual_norm()
+    assert abs(rel - rel2) <= 1e-12 * rel2 and rel <= tol
+    assert abs(final - onorms[done]) <= (1e-5 if cfg.dtype == "f32" else 1e-10) * onorms[done]
+    # the same cycles issued one by one give the same u, bit for bit
+    r = mk()
+    r.cycle(done)
+    assert np.array_equal(r.get_solution(), u)
+    assert r.residual_history() == hist
+    # the cap stops the loop; solving on continues from where it is; homg_cycle after homg_solve appends
+    t = mk()
+    d1, rel1 = t.solve(tol, 2)
+    assert d1 == 2 and rel1 > tol
+    d2, _ = t.solve(tol, cap)
+    assert d1 + d2 == want and np.array_equal(t.get_solution(), u)
+    d3, _ = t.solve(tol, cap)
+    assert d3 == 0                                                      # already converged: no cycle runs
+    t.cycle(1)
+    assert len(t.residual_history()) == want + 1
+    r.cycle(1)
+    assert np.array_equal(t.get_solution(), r.get_solution())
+    assert t.residual_history() == r.residual_history()
+    for x in (s, r, t):
+        x.destroy()
+
+
+def test_solve_argument_checks():
+    _torch()
+    from paper_1108_2045_b200 import homg
+    s = homg.Solver((17, 17), 3, "poisson5", "f64")
+    with pytest.raises(homg.HomgError) as ei:
+        s.solve(1e-8, 10)
+    assert ei.value.status == homg.HOMG_ESTATE
+    s.set_rhs(np.ones((17, 17)))
+    with pytest.raises(homg.HomgError):
+        s.solve(-1.0, 10)
+    with pytest.raises(homg.HomgError):
+        s.solve(1e-8, 5000)                                             # history_cap (4096) too small
+    assert s.solve(1e-8, 0)[0] == 0
+    s.destroy()
+    v = homg.Solver((17, 17), 4, "poisson5", "f64", vcycle=(2, 1))
+    v.set_rhs(np.ones((17, 17)))
+    with pytest.raises(homg.HomgError) as ei:
+        v.solve(1e-8, 10)
+    assert ei.value.status == homg.HOMG_ESTATE
+    v.destroy()
 
 
 # ---- mixed-precision outer loop (SURVEY.md 8(f)2) vs the oracle's mixed loop: fp64 u, f, r; fp32 correction cycle ----
