@@ -1,16 +1,18 @@
 #!/usr/bin/env python
 """bench.py — HOMG solve throughput on B200 (driver contract: one JSON line on stdout from rank 0).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl reference]
 
-A "step" is one whole solve of the workload: reset u <- u0, c* outer HOMG cycles (residual ->
-restriction -> MFMG visits -> u += e; c* = cycles the solve needs to reach the config's relative
-residual, found once during warm-up from the device-side norm history), and the final residual norm.
+A "step" is one whole solve of the workload through homg_solve: reset u <- u0, then outer HOMG cycles
+(residual -> restriction -> MFMG visits -> u += e) repeated ON THE DEVICE until the config's relative residual
+is reached — the cycle count is decided by the solve itself, not learnt beforehand.
   value        fine-grid unknowns solved per second, inputs resident in HBM (device-timed, CUDA events)
-  e2e          the same through the C ABI with HOST buffers (pinned): H2D of f and u0, the solve, D2H of u
-  roofline     the dominant kernel (level-0 Jacobi sweep), timed live with CUDA events per launch
-  cpu_baseline the oracle (oracle/, Algorithm H, single thread) on a bounded sample of the same solve
-N > 1: independent replicas, one per GPU ("replicas only": the path has no exchange step).
+  e2e          the same through the C ABI with HOST buffers (pinned): H2D of f (u0, k), the solve, D2H of u
+  roofline     the level-0 kernel class with the largest share of the cycle, timed live with CUDA events per launch;
+               achieved = the bytes the launch itself must move / its duration
+  cpu_baseline the oracle (oracle/, Algorithm H, single thread, untuned) on a bounded sample of the same workload
+Default workload: cfg4 (513^3 fp32, 540 MB per array — HBM-resident; north_star quotes its bandwidth target on
+it).  N > 1: independent replicas, one per GPU ("replicas only": the path has no exchange step).
 """
 import argparse
 import json
@@ -38,7 +40,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="homg", choices=["homg", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=sorted(I.CONFIGS))
+    ap.add_argument("--workload", default="cfg4", choices=sorted(I.CONFIGS))
     ap.add_argument("--n", type=int, default=0, help="scale the workload to an n^d grid (debugging)")
     ap.add_argument("--cycle", default="mfmg", choices=["mfmg", "v", "literal"],
                     help="mfmg: the paper's HOMG cycle (default); v: classic V(2,1) on the same kernels; "
@@ -48,19 +50,21 @@ def parse():
                          "fp32; the workload's inputs are generated in fp64 (cfg3/cfg4: makes tolerances below the "
                          "fp32 floor reachable; cfg2/cfg5: halves the sweep traffic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the largest-3-D-grid roofline pass")
+    ap.add_argument("--no-extra", action="store_true", help="skip the side rows (classic V(2,1), paper-literal mode)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
+    ap.add_argument("--ref-seconds", type=float, default=120.0, help="--impl reference: budget of the whole run")
     return ap.parse_args()
 
 
-def workload_config(cfg):
+def workload_config(cfg, cycle="mfmg"):
+    stop = f"stop rel. residual {cfg.tol:g}" if cfg.tol > 0 else f"{cfg.cycles} cycles"
     return {"workload": f"{cfg.name}: {'x'.join(map(str, cfg.dims))} nodes, {cfg.dtype}, {cfg.levels} levels, "
-                        f"{cfg.stencil}, omega={cfg.omega:.6g}, MFMG schedule C MaxI={cfg.max_iters}, "
-                        f"stop rel. residual {cfg.tol:g}" if cfg.tol > 0 else
-                        f"{cfg.name}: {'x'.join(map(str, cfg.dims))} nodes, {cfg.dtype}, {cfg.levels} levels, "
-                        f"{cfg.stencil}, omega={cfg.omega:.6g}, MFMG schedule C MaxI={cfg.max_iters}, {cfg.cycles} cycles",
+                        f"{cfg.stencil}, omega={cfg.omega:.6g}, MFMG schedule C MaxI={cfg.max_iters}, {stop}",
             "dims": list(cfg.dims), "levels": cfg.levels, "stencil": cfg.stencil, "tol": cfg.tol,
-            "parallelism": "replicas only (one independent solve per GPU)"}
+            "parallelism": "replicas only (one independent solve per GPU)",
+            "l2": "flushed between steps (512 MiB write); level-0 arrays of cfg3-5 are larger than L2",
+            "cycle": {"mfmg": "MFMG (HOMG), per-level arrays", "v": "classic V(2,1)",
+                      "literal": "MFMG (HOMG), paper-literal whole-grid iteration"}[cycle]}
 
 
 def peaks():
@@ -114,22 +118,10 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def cycles_to_tol(hist_plus_final, cfg):
-    """first c such that ||r_c|| / ||r_0|| <= tol (norm BEFORE cycle c == after cycle c-1); fixed count if tol == 0."""
-    if cfg.tol <= 0:
-        return cfg.cycles, None
-    n0 = hist_plus_final[0]
-    for c, v in enumerate(hist_plus_final):
-        if v <= cfg.tol * n0:
-            return c, v / n0
-    return None, min(hist_plus_final) / n0
-
-
 def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False, mixed=False):
     from paper_1108_2045_b200 import homg
     s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters,
                     schedule=cfg.schedule, device=dev, vcycle=vcycle, literal=literal, mixed=mixed)
-    tdt = torch.float64 if cfg.dtype == "f64" else torch.float32
     d = {k: (None if v is None else torch.from_numpy(v).to(dev)) for k, v in inp.items()}
     if not inp["u0"].any():
         d["u0"] = None          # the config's u0 = 0 is the library's default guess: set_initial_guess(None), no array
@@ -137,137 +129,160 @@ def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False, mixed=False):
         s.set_coefficient(d["k"])
     s.set_rhs(d["f"])
     s.set_initial_guess(d["u0"])
-    return s, d, tdt
+    return s, d
 
 
-def find_cstar(s, d, cfg):
-    """runs the capped cycle count once and reads the history back (outside any timed region)."""
-    s.set_initial_guess(d["u0"])
-    s.cycle(cfg.cycles)
-    hist = s.residual_history()
-    final, _ = s.residual_norm()
-    c, rel = cycles_to_tol(hist + [final], cfg)
-    stagnated = c is None
-    if stagnated:      # tolerance below the arithmetic's floor (DESIGN.md R17): stop where the norm stops falling
-        allv = hist + [final]
-        c = int(np.argmin(allv))
-    return max(1, c), rel, stagnated, (hist + [final])
+class Solve:
+    """one solve of the workload = one bench step.  MFMG: homg_solve (the device-side loop stops by itself; a config
+    without a tolerance runs its fixed cycle count).  Side rows (classic V, paper-literal, mixed precision) have no
+    homg_solve: they run the cycle count a first run of the same solve needed (find_cstar)."""
+
+    def __init__(self, s, cfg, own_loop):
+        self.s, self.cfg, self.own_loop, self.cstar = s, cfg, own_loop, None
+
+    def find_cstar(self, u0):
+        cfg, s = self.cfg, self.s
+        s.set_initial_guess(u0)
+        s.cycle(cfg.cycles)
+        allv = s.residual_history() + [s.residual_norm()[0]]
+        c = next((i for i, v in enumerate(allv) if v <= cfg.tol * allv[0]), None) if cfg.tol > 0 else cfg.cycles
+        self.cstar = max(1, int(np.argmin(allv)) if c is None else c)
+        return self.cstar
+
+    def run(self, u0):
+        """-> (cycles, final relative residual)"""
+        cfg, s = self.cfg, self.s
+        s.set_initial_guess(u0)
+        if self.own_loop and cfg.tol > 0:
+            return s.solve(cfg.tol, cfg.cycles)
+        n = self.cstar if self.cstar is not None else cfg.cycles
+        s.cycle(n)
+        return n, s.residual_norm()[1]
 
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from `ncu --set full`
-# captures, one launch each; the summaries and their commands are under profiles/.
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from `ncu --set full` captures, one launch
+# each; the summaries and their commands are under profiles/ (the tag names the capture, so a stale entry shows).
 NCU_TRAFFIC = {
-    ("cfg4", "visit_l0"): (1.318703e9 + 0.514103e9, "profiles/r01e_ncu_full_cfg4.md"),
-    ("cfg4", "residual_l0"): (1.152890e9 + 0.571569e9, "profiles/r01e_ncu_full_cfg4.md"),
-    ("cfg4", "relax_l0"): (1.164186e9 + 0.509018e9, "profiles/r01b_ncu_full_cfg4.md"),
-    ("cfg2", "visit_l0"): (43.483904e6 + 0.012800e6, "profiles/r01d_ncu_full_cfg2.md"),      # L2-resident (17 MB arrays)
-    ("cfg2", "residual_l0"): (36.909056e6 + 0.042752e6, "profiles/r01d_ncu_full_cfg2.md"),
-    ("cfg3", "visit_l0"): (693.390848e6 + 235.526656e6, "profiles/r01e_ncu_full_cfg3.md"),
-    ("cfg3", "residual_l0"): (548.102656e6 + 302.414592e6, "profiles/r01e_ncu_full_cfg3.md"),
-    ("cfg5", "relax_l0"): (687.057920e6 + 121.797120e6, "profiles/r01e_ncu_full_cfg5.md"),
-    ("cfg5", "relax_l0_last"): (821.715712e6 + 122.345984e6, "profiles/r01e_ncu_full_cfg5.md"),
-    ("cfg5", "residual_l0"): (690.258176e6 + 137.026304e6, "profiles/r01e_ncu_full_cfg5.md"),
+    ("cfg4", "visit_l0"): (1.301990e9 + 0.512010e9, "profiles/r02a_ncu_full_cfg4.md"),
+    ("cfg4", "residual_l0"): (1.152890e9 + 0.571569e9, "profiles/r01e_ncu_full_cfg4.md (kernel unchanged since)"),
+    ("cfg3", "visit_l0"): (693.390848e6 + 235.526656e6, "profiles/r01e_ncu_full_cfg3.md (kernel unchanged since)"),
+    ("cfg3", "residual_l0"): (548.102656e6 + 302.414592e6, "profiles/r01e_ncu_full_cfg3.md (kernel unchanged since)"),
+    ("cfg5", "relax_l0"): (687.057920e6 + 121.797120e6, "profiles/r01e_ncu_full_cfg5.md (kernel unchanged since)"),
+    ("cfg5", "relax_l0_last"): (821.715712e6 + 122.345984e6, "profiles/r01e_ncu_full_cfg5.md (kernel unchanged since)"),
+    ("cfg5", "residual_l0"): (690.258176e6 + 137.026304e6, "profiles/r01e_ncu_full_cfg5.md (kernel unchanged since)"),
 }
 LEVEL0_CLASSES = ("visit_l0", "relax_l0", "relax_l0_first", "relax_l0_last", "residual_l0")
 
 
-def roofline_from_profile(prof, peak, peak_src, comp=None, cycles=1, wname=""):
-    """roofline of the level-0 kernel class that takes the most time (K_visit = the fused
-    interpolate+correct+relax visit when it runs): achieved = ALGORITHMIC bytes (3 arrays
-    per Jacobi node-update, (2+2/2^d) for the first sweep of a visit, 4 for the one that adds u) over the
-    event-timed duration.  K_visit performs the sweeps of a visit in one pass, so its COMPULSORY bytes
-    (what the launch itself must move) are reported next to it; `traffic` is the ncu DRAM byte count."""
+def roofline_from_profile(prof, peak, peak_src, comp, cycles, wname):
+    """Per kernel class (CUDA events after every launch, homg_profile_cycles): duration, share of the cycle and
+      hbm_gbs        = the bytes the launches themselves must move ("compulsory": every array a launch reads or
+                       writes, once; DESIGN.md 8) / duration — the HBM roofline number, frac = hbm_gbs / peak;
+      sweep_equiv_gbs = SURVEY.md 8(d)'s per-sweep count (3 arrays per Jacobi node-update) / duration: equal to
+                       hbm_gbs for single-operation kernels, larger for K_visit, which runs the eta sweeps of a
+                       visit in one pass (it may exceed the HBM peak; it is not a bandwidth).
+    `roofline` = the level-0 class with the largest share."""
     if not prof:
         return None, {}
-    comp = comp or {}
     total_ms = sum(v[0] for v in prof.values())
-    l0 = [k for k in prof if k in LEVEL0_CLASSES]
-    name = max(l0 or prof, key=lambda k: prof[k][0])
     shares = {}
     for k, v in prof.items():
         cb = comp.get(k, 0.0) * cycles
+        tr = NCU_TRAFFIC.get((wname, k))
+        sec = v[0] * 1e-3
         shares[k] = {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / total_ms,
-                     "algorithmic_gbs": (v[2] / (v[0] * 1e-3) / 1e9) if v[0] > 0 else 0.0,
-                     "compulsory_gbs": (cb / (v[0] * 1e-3) / 1e9) if v[0] > 0 else 0.0}
-    ms, cnt, by = prof[name]
-    ach = by / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
-    cb = comp.get(name, 0.0) * cycles
+                     "hbm_gbs": cb / sec / 1e9 if sec > 0 else 0.0, "frac_of_peak": cb / sec / 1e9 / peak if sec > 0 else 0.0,
+                     "bytes_per_launch": cb / v[1], "sweep_equiv_gbs": v[2] / sec / 1e9 if sec > 0 else 0.0,
+                     "ncu_dram_bytes_per_launch": tr[0] if tr else None}
+    l0 = [k for k in prof if k in LEVEL0_CLASSES]
+    name = max(l0 or prof, key=lambda k: prof[k][0])
+    k = shares[name]
     tr = NCU_TRAFFIC.get((wname, name))
-    rl = {"bound": "hbm", "kernel": name, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-          "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
-          "peak_source": peak_src, "ms_per_launch": ms / cnt, "launches": cnt,
-          "bytes_per_launch": by / cnt, "compulsory_bytes_per_launch": cb / cnt,
-          "compulsory_gbs": cb / (ms * 1e-3) / 1e9 if ms > 0 else 0.0,
-          "share_of_cycle": ms / total_ms, "frac_of_8TBs_nominal": ach / 8000.0,
-          "note": "achieved counts the per-sweep algorithmic bytes of SURVEY.md 8(d); a fused multi-sweep "
-                  "launch (visit_l0) moves only compulsory_bytes_per_launch, so achieved may exceed the HBM peak"}
+    rl = {"bound": "hbm", "kernel": name, "achieved": k["hbm_gbs"], "peak": peak, "unit": "GB/s", "frac": k["frac_of_peak"],
+          "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None, "peak_source": peak_src,
+          "ms_per_launch": k["ms_per_launch"], "launches": k["launches"], "bytes_per_launch": k["bytes_per_launch"],
+          "share_of_cycle": k["share"], "frac_of_8TBs_nominal": k["hbm_gbs"] / 8000.0,
+          "sweep_equiv_gbs": k["sweep_equiv_gbs"],
+          "note": "achieved = bytes the launch itself must move / CUDA-event duration. visit_l0 (interpolate+correct + "
+                  "4 sweeps + u += e in one pass) is bound by instruction issue and shared-memory bandwidth, not by "
+                  "HBM (profiles/): its frac is what is left to the HBM floor; sweep_equiv_gbs counts the per-sweep "
+                  "bytes of SURVEY.md 8(d) and is not a bandwidth"}
     return rl, shares
 
 
-def cpu_baseline(cfg, inp, cstar, seconds):
-    """the oracle as it stands (Algorithm H, one thread) on the first cycles of the same solve."""
+def sample_config(cfg, seconds_per_solve):
+    """the workload's recipe at the largest n^d grid (n = 2^j + 1, at most the workload's own) whose oracle solve is
+    estimated to fit `seconds_per_solve`: the oracle's cost is linear in the nodes (pin P10)."""
+    from oracle import oracle as O
+    nd = len(cfg.dims)
+    small = I.scaled(cfg, 33 if nd == 3 else 257)
+    inp = I.make_inputs(small)
+    sched = O.schedule(small.schedule, small.levels, small.max_iters)
+    O.homg("H", inp["f"], inp["u0"], small.levels, small.omega, sched, 1, k=inp["k"], keep_history=False)     # warm
+    t0 = time.perf_counter()
+    O.homg("H", inp["f"], inp["u0"], small.levels, small.omega, sched, 2, k=inp["k"], keep_history=False)
+    per_node_cycle = (time.perf_counter() - t0) / 2 / float(np.prod(small.dims))
+    est_cycles = 12 if cfg.tol > 0 else cfg.cycles
+    n = cfg.dims[0]
+    while n > (33 if nd == 3 else 257) and per_node_cycle * float(n) ** nd * est_cycles > seconds_per_solve:
+        n = (n - 1) // 2 + 1
+    return cfg if n == cfg.dims[0] else I.scaled(cfg, n)
+
+
+def oracle_solve(cfg, inp):
+    """one complete solve by the oracle as it stands (Algorithm H, one thread): cycles until the tolerance, as
+    homg_solve does.  -> (seconds, cycles, relative residual)"""
     from oracle import oracle as O
     sched = O.schedule(cfg.schedule, cfg.levels, cfg.max_iters)
     u = inp["u0"].copy()
-    t_used, ncyc = 0.0, 0
-    while ncyc < cstar and (ncyc == 0 or t_used + t_used / ncyc <= seconds):
-        t0 = time.perf_counter()
-        u, _, _ = O.homg("H", inp["f"], u, cfg.levels, cfg.omega, sched, 1, k=inp["k"], keep_history=False)
-        t_used += time.perf_counter() - t0
-        ncyc += 1
-    t_cycle = t_used / ncyc
-    return {"value": cfg.n_interior / (t_cycle * cstar), "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"first {ncyc} of {cstar} cycles of the same solve ({t_used:.1f} s), scaled to {cstar} cycles",
-            "s_per_cycle": t_cycle, "host_cores_available": os.cpu_count()}
+    t0 = time.perf_counter()
+    n0, rel, c = None, 1.0, 0
+    while c < cfg.cycles:
+        u, _, n = O.homg("H", inp["f"], u, cfg.levels, cfg.omega, sched, 1, k=inp["k"], keep_history=False)
+        n0 = n[0] if n0 is None else n0
+        c += 1
+        rel = n[1] / n0 if n0 > 0 else 0.0
+        if cfg.tol > 0 and rel <= cfg.tol:
+            break
+    return time.perf_counter() - t0, c, rel
+
+
+def cpu_baseline(cfg, seconds):
+    scfg = sample_config(cfg, seconds)
+    sec, cyc, rel = oracle_solve(scfg, I.make_inputs(scfg))
+    return {"value": scfg.n_interior / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"one complete solve of the same recipe at {'x'.join(map(str, scfg.dims))} ({cyc} cycles to rel. residual "
+                      f"{rel:.2e}, {sec:.1f} s); the oracle is single-threaded, untuned test infrastructure (-O2, no SIMD "
+                      f"pragmas), cost linear in the nodes",
+            "host_cores_available": os.cpu_count()}
 
 
 def run_reference(args):
-    """--impl reference: the oracle (CPU, one thread) on the same workload.  Rank 0 only."""
+    """--impl reference: the oracle (CPU, one thread, as it stands) on a bounded sample of the workload; every step is
+    one COMPLETE, fully timed solve.  Rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    from oracle import oracle as O
     cfg = I.CONFIGS[args.workload]
     if args.n:
         cfg = I.scaled(cfg, args.n)
-    inp = I.make_inputs(cfg)
-    sched = O.schedule(cfg.schedule, cfg.levels, cfg.max_iters)
-    budget = 150.0
-    # warm-up: cycles until the tolerance (bounded) -> c*; t_cycle estimate
-    t0 = time.perf_counter()
-    u = inp["u0"].copy()
-    norms, cstar = [], None
-    for c in range(cfg.cycles):
-        u, _, n = O.homg("H", inp["f"], u, cfg.levels, cfg.omega, sched, 1, k=inp["k"], keep_history=False)
-        if c == 0:
-            norms.append(n[0])
-        norms.append(n[1])
-        if cfg.tol > 0 and n[1] <= cfg.tol * norms[0]:
-            cstar = c + 1
-            break
-        if time.perf_counter() - t0 > budget / 3:
-            break
-    done = len(norms) - 1
-    t_cycle0 = (time.perf_counter() - t0) / done
-    known = {"cfg2": 14, "cfg3": 7, "cfg4": 9, "cfg5": 20}      # SURVEY.md A.2 probe counts, used only if the
-    if cstar is None:                                           # bounded warm-up did not reach the tolerance
-        cstar = cfg.cycles if cfg.tol <= 0 else known.get(cfg.name.split("@")[0], done)
-    per_step = max(1, min(cstar, int((budget * 2 / 3) / max(1, args.steps) / t_cycle0)))
-    t_sum = 0.0
+    warm = max(1, args.warmup)
+    scfg = sample_config(cfg, args.ref_seconds / (args.steps + warm))
+    inp = I.make_inputs(scfg)
+    for _ in range(warm):
+        oracle_solve(scfg, inp)
+    t_sum, cyc, rel = 0.0, 0, 1.0
     for _ in range(args.steps):
-        u = inp["u0"].copy()
-        t1 = time.perf_counter()
-        O.homg("H", inp["f"], u, cfg.levels, cfg.omega, sched, per_step, k=inp["k"], keep_history=False)
-        t_sum += time.perf_counter() - t1
-    t_cycle = t_sum / (args.steps * per_step)
-    t_solve = t_cycle * cstar
-    val = cfg.n_interior / t_solve
-    sample = f"{per_step} of {cstar} cycles per step, scaled to {cstar} cycles"
+        sec, cyc, rel = oracle_solve(scfg, inp)
+        t_sum += sec
+    val = scfg.n_interior * args.steps / t_sum
+    sample = (f"every step = one complete solve of the same recipe at {'x'.join(map(str, scfg.dims))} "
+              f"({cyc} cycles to rel. residual {rel:.2e}), timed in full")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": t_solve * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": t_sum / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic", "config": workload_config(cfg),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "cycles_to_tol": cstar, "gpu_launches": 0}
+            "cycles_to_tol": cyc, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
@@ -288,17 +303,15 @@ def run_homg(args):
         import dataclasses
         cfg = dataclasses.replace(cfg, dtype="f64")
     inp = I.make_inputs(cfg)
-    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None,
-                          literal=args.cycle == "literal", mixed=args.mixed)
-    cstar, rel, stagnated, norms = find_cstar(s, d, cfg)
+    own_loop = args.cycle == "mfmg" and not args.mixed
+    s, d = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None,
+                       literal=args.cycle == "literal", mixed=args.mixed)
+    job = Solve(s, cfg, own_loop)
+    if not (own_loop and cfg.tol > 0) and cfg.tol > 0:
+        job.find_cstar(d["u0"])
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     sampler = ClockSampler(local)
     stream = torch.cuda.current_stream()
-
-    def step_dev():
-        s.set_initial_guess(d["u0"])
-        s.cycle(cstar)
-        return s.residual_norm()
 
     def sync_all():
         torch.cuda.synchronize()
@@ -307,20 +320,21 @@ def run_homg(args):
 
     for _ in range(max(3, args.warmup)):
         flush.zero_()
-        step_dev()
+        job.run(d["u0"])
     sync_all()
     t_a = time.time()
-    total_ms = 0.0
+    total_ms, cycles, rel = 0.0, 0, 1.0
     for _ in range(args.steps):
         flush.zero_()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        final = step_dev()
+        cycles, rel = job.run(d["u0"])
         e1.record(stream)
         e1.synchronize()
         total_ms += e0.elapsed_time(e1)
     sync_all()
     sampler.mark(t_a, time.time())
+    stagnated = cfg.tol > 0 and rel > cfg.tol
 
     # ---- e2e: host buffers through the C ABI ----
     hf = torch.from_numpy(inp["f"]).pin_memory()
@@ -332,9 +346,7 @@ def run_homg(args):
         if hk is not None:
             s.set_coefficient(hk)
         s.set_rhs(hf)
-        s.set_initial_guess(hu0)
-        s.cycle(cstar)
-        r = s.residual_norm()
+        r = job.run(hu0)
         s.get_solution(hout)
         return r
 
@@ -355,46 +367,46 @@ def run_homg(args):
     sampler.mark(t_b, time.time())
 
     # ---- per-kernel timing (CUDA events after every launch, plain stream launches) ----
+    launches_cycle = s.launches_per_cycle()
     prof = {}
     if not args.mixed:                          # (homg_profile_cycles is not available in mixed precision)
         s.set_initial_guess(d["u0"])
         s.profile_cycles(1)                     # warm
         s.set_initial_guess(d["u0"])
         t_c = time.time()
-        prof = s.profile_cycles(cstar)
+        prof = s.profile_cycles(cycles)
         sampler.mark(t_c, time.time())
     peak, peak_src = peaks()
     comp, comp_total = s.compulsory_bytes_per_cycle()
-    rl, shares = roofline_from_profile(prof, peak, peak_src, comp, cstar, cfg.name)
-    launches_step = s.launches_per_cycle() * cstar + (2 if d["u0"] is not None else 0) + 2   # + pack(u0) (u0 = 0: a memset, not counted) + norm-only pass (2 kernels)
+    rl, shares = roofline_from_profile(prof, peak, peak_src, comp, cycles, cfg.name)
+    # kernels of one step: the cycles + the first residual pass of homg_solve (2 kernels) or the closing norm-only
+    # pass (2) + the pack of u0 (1; u0 = 0 is a memset)
+    launches_step = launches_cycle * cycles + 2 + (1 if d["u0"] is not None else 0)
     bytes_cycle = s.bytes_per_cycle()
     clocks = sampler.stop()
 
     total_ms, e2e_s = replicas.max_over_ranks([total_ms, e2e_s], device=dev)
     es = 8 if cfg.dtype == "f64" else 4
     nbytes = int(np.prod(cfg.dims)) * es
+    ms_cycle = total_ms / args.steps / max(cycles, 1)
     line = {"metric": METRIC, "value": replicas.job_value(cfg.n_interior, args.steps, world, total_ms), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64 (u, f, residual) / f32 (correction cycle)" if args.mixed else cfg.dtype, "data": "synthetic",
-            "config": dict(workload_config(cfg), l2="flushed between steps (512 MiB write)",
-                           cycle={"mfmg": "MFMG (HOMG), per-level arrays", "v": "classic V(2,1)",
-                                  "literal": "MFMG (HOMG), paper-literal whole-grid iteration"}[args.cycle]),
-            "cycles_to_tol": cstar, "rel_residual_reached": float(final[1]), "stagnated_above_tol": bool(stagnated),
-            "ms_per_cycle": total_ms / args.steps / cstar,
-            "unknowns_per_s_per_cycle": cfg.n_interior * world / (total_ms * 1e-3 / args.steps / cstar),
-            "cycle_algorithmic_gb": bytes_cycle / 1e9,
-            "cycle_algorithmic_gbs": bytes_cycle / (total_ms * 1e-3 / args.steps / cstar) / 1e9,
-            "cycle_compulsory_gb": comp_total / 1e9,
-            "cycle_compulsory_gbs": comp_total / (total_ms * 1e-3 / args.steps / cstar) / 1e9,
+            "config": workload_config(cfg, args.cycle),
+            "cycles_to_tol": cycles, "cycles_decided_by": "homg_solve (device-side loop)" if own_loop and cfg.tol > 0 else
+            ("fixed by the config" if cfg.tol <= 0 else "a first run of the same solve"),
+            "rel_residual_reached": float(rel), "stagnated_above_tol": bool(stagnated),
+            "ms_per_cycle": ms_cycle, "unknowns_per_s_per_cycle": cfg.n_interior * world / (ms_cycle * 1e-3),
+            "cycle_sweep_equiv_gb": bytes_cycle / 1e9, "cycle_hbm_gb": comp_total / 1e9,
+            "cycle_hbm_gbs": comp_total / (ms_cycle * 1e-3) / 1e9, "cycle_hbm_frac_of_peak": comp_total / (ms_cycle * 1e-3) / 1e9 / peak,
             "e2e": {"value": cfg.n_interior * n_e2e * world / e2e_s, "unit": UNIT, "ms_per_step": e2e_s / n_e2e * 1e3,
-                    "h2d_bytes_per_step": nbytes * (1 + (hk is not None) + (hu0 is not None)), "d2h_bytes_per_step": nbytes + 8},
-            "gpu_launches": launches_step * args.steps, "roofline": rl, "kernels": shares, "clocks": clocks}
+                    "h2d_bytes_per_step": nbytes * (1 + (hk is not None) + (hu0 is not None)), "d2h_bytes_per_step": nbytes + 20},
+            "gpu_launches": launches_step * args.steps, "launches_per_cycle": launches_cycle, "roofline": rl, "kernels": shares,
+            "clocks": clocks}
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(cfg, inp, cstar, args.cpu_seconds)
-        if not args.no_extra and world == 1 and not args.n and args.workload != "cfg4" and not args.mixed:
-            line["roofline_largest_3d"] = extra_largest(torch, dev, peak, peak_src)
+            line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_seconds)
         if not args.no_extra and world == 1 and args.cycle == "mfmg" and not args.mixed:
             line["classic_v21"] = extra_other(torch, dev, cfg, inp, flush, vcycle=(2, 1))
             line["paper_literal"] = extra_other(torch, dev, cfg, inp, flush, literal=True)
@@ -408,51 +420,47 @@ def extra_other(torch, dev, cfg, inp, flush, vcycle=None, literal=False):
     """the same solve with another cycle on the same hierarchy and operators: the classic V(2,1) cycle — the
     comparison the paper argues — or the paper's own whole-grid design (Algorithm L:
     one fine-grid array, one whole-grid launch per iteration, L51/L119), which the per-level layout replaces."""
-    s, d, _ = make_solver(cfg, inp, torch, dev, vcycle=vcycle, literal=literal)
-    cstar, rel, stagnated, _ = find_cstar(s, d, cfg)
-    reps = 2 if literal else 5
-    for _ in range(1 if literal else 3):
-        s.set_initial_guess(d["u0"]); s.cycle(cstar); s.residual_norm()
-    ms = 0.0
+    s, d = make_solver(cfg, inp, torch, dev, vcycle=vcycle, literal=literal)
+    job = Solve(s, cfg, False)
+    if literal and cfg.n_interior > 3e7:        # (seconds per solve: one capped probe of the cycle count is all it gets)
+        import dataclasses
+        job.cfg = dataclasses.replace(cfg, cycles=min(cfg.cycles, 12))
+    cstar = job.find_cstar(d["u0"]) if cfg.tol > 0 else cfg.cycles
+    reps = 1 if literal else 5
+    for _ in range(0 if literal else 2):
+        job.run(d["u0"])
+    ms, fin = 0.0, 1.0
     for _ in range(reps):
         flush.zero_()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record()
-        s.set_initial_guess(d["u0"]); s.cycle(cstar); fin = s.residual_norm()
+        _, fin = job.run(d["u0"])
         e1.record(); e1.synchronize()
         ms += e0.elapsed_time(e1)
     ms /= reps
     out = {"cycles_to_tol": cstar, "ms_per_step": ms, "ms_per_cycle": ms / cstar, "value": cfg.n_interior / (ms * 1e-3),
-           "unit": UNIT, "rel_residual_reached": float(fin[1]), "stagnated_above_tol": bool(stagnated),
+           "unit": UNIT, "rel_residual_reached": float(fin), "stagnated_above_tol": bool(cfg.tol > 0 and fin > cfg.tol),
            "launches_per_cycle": s.launches_per_cycle()}
     s.destroy()
     return out
 
 
-def extra_largest(torch, dev, peak, peak_src):
-    """north_star's bandwidth target is quoted on the largest 3-D grid (cfg4, 513^3 fp32): per-kernel
-    event timing of a few cycles there (arrays of 540 MB, far larger than L2)."""
-    cfg = I.CONFIGS["cfg4"]
-    inp = I.make_inputs(cfg)
-    s, d, _ = make_solver(cfg, inp, torch, dev)
-    s.cycle(2)
-    torch.cuda.synchronize()
-    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    e0.record(); s.cycle(5); e1.record(); e1.synchronize()
-    ms_cycle = e0.elapsed_time(e1) / 5
-    prof = s.profile_cycles(3)
-    comp, _ = s.compulsory_bytes_per_cycle()
-    rl, shares = roofline_from_profile(prof, peak, peak_src, comp, 3, cfg.name)
-    out = {"workload": workload_config(cfg)["workload"], "ms_per_cycle_graph": ms_cycle,
-           "unknowns_per_s_per_cycle": cfg.n_interior / (ms_cycle * 1e-3),
-           "cycle_algorithmic_gbs": s.bytes_per_cycle() / (ms_cycle * 1e-3) / 1e9, "dominant": rl, "kernels": shares}
-    s.destroy()
-    return out
+def spawn_replicas(args):
+    """`python bench.py --gpus N` outside torchrun: launch the N replicas ourselves (one process per GPU)."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_replicas(a)
     else:
         run_homg(a)
