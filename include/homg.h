@@ -175,6 +175,11 @@ HOMG_API homg_status homg_get_solution(homg_solver* s, void* dst, int on_device)
  * (DESIGN.md "Roofline"). */
 HOMG_API int homg_get_schedule(const homg_solver* s, int* levels_out, int* iters_out, int cap);
 HOMG_API int homg_launches_per_cycle(const homg_solver* s);
+/* Node census of the CUDA graph homg_cycle replays (which = 0) or of the graph homg_solve launches, its loop body
+ * included (which = 1): counts[0..4] = kernel, memset, memcpy, conditional (WHILE), other nodes.  Evidence for "no
+ * host transfers inside a solve": memcpy and other (host, event, ...) are 0.  HOMG_ESTATE before the first
+ * homg_cycle / homg_solve. */
+HOMG_API homg_status homg_graph_nodes(const homg_solver* s, int which, int* counts);
 HOMG_API double homg_bytes_per_cycle(const homg_solver* s, int level0_only);
 
 /* Measurement aid (bench.py): runs n cycles with plain stream launches and a CUDA event after every

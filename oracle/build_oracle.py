@@ -17,8 +17,18 @@ CMD = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-ffp-contract=off", "-o"
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
-        subprocess.check_call(CMD)
+    """HOMG_ORACLE_CFLAGS (e.g. "-fsanitize=undefined -fno-sanitize-recover=all -g") adds flags for a one-off checked
+    build (profiles/r02_sanitizer.md); such a build is always redone, and so is the next plain one."""
+    extra = os.environ.get("HOMG_ORACLE_CFLAGS", "").split()
+    stamp = LIB + ".flags"
+    last = open(stamp).read() if os.path.exists(stamp) else ""
+    if force or extra or last or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
+        subprocess.check_call(CMD[:-3] + extra + CMD[-3:])
+        if extra:
+            with open(stamp, "w") as fh:
+                fh.write(" ".join(extra))
+        elif os.path.exists(stamp):
+            os.remove(stamp)
     return LIB
 
 

@@ -40,6 +40,25 @@ void drop_graph(homg_solver* s) {
     if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
     if (s->solve_exec) { cudaGraphExecDestroy(s->solve_exec); s->solve_exec = nullptr; }
     if (s->solve_graph) { cudaGraphDestroy(s->solve_graph); s->solve_graph = nullptr; }
+    s->solve_body = nullptr;
+}
+
+cudaError_t census(cudaGraph_t g, int* c) {
+    size_t n = 0;
+    cudaError_t e = cudaGraphGetNodes(g, nullptr, &n);
+    if (e != cudaSuccess) return e;
+    std::vector<cudaGraphNode_t> nodes(n + 1);
+    if (n && (e = cudaGraphGetNodes(g, nodes.data(), &n)) != cudaSuccess) return e;
+    for (size_t i = 0; i < n; ++i) {
+        cudaGraphNodeType t;
+        if ((e = cudaGraphNodeGetType(nodes[i], &t)) != cudaSuccess) return e;
+        if (t == cudaGraphNodeTypeKernel) ++c[0];
+        else if (t == cudaGraphNodeTypeMemset) ++c[1];
+        else if (t == cudaGraphNodeTypeMemcpy) ++c[2];
+        else if (t == cudaGraphNodeTypeConditional) ++c[3];
+        else ++c[4];
+    }
+    return cudaSuccess;
 }
 
 struct SolveParamsHost { double tol2; int max_slot; int pad; };   // = SolveParams of homg_kernels.cuh
@@ -66,6 +85,8 @@ homg_status build_solve_graph(homg_solver* s) {
     if (ne) CU(s, cudaGraphGetEdges(s->solve_graph, from.data(), to.data(), &ne));
     std::vector<cudaGraphNode_t> leaves;
     for (auto n : nodes) if (std::find(from.begin(), from.end(), n) == from.end()) leaves.push_back(n);
+    for (int i = 0; i < 5; ++i) s->solve_census[i] = 0;
+    CU(s, census(s->solve_graph, s->solve_census));              // the prologue (before the WHILE node exists)
     cudaGraphNodeParams p = {};
     p.type = cudaGraphNodeTypeConditional;
     p.conditional.handle = h;
@@ -75,11 +96,14 @@ homg_status build_solve_graph(homg_solver* s) {
     e = cudaGraphAddNode(&cn, s->solve_graph, leaves.data(), leaves.size(), &p);
     if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: conditional node"); }
     cudaGraph_t body = p.conditional.phGraph_out[0];
+    s->solve_body = body;
     e = cudaStreamBeginCaptureToGraph(s->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
     if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: graph body"); }
     e = exec_solve_body(s, s->cap_stream, (unsigned long long)h);
     e2 = cudaStreamEndCapture(s->cap_stream, &got);
     if (e != cudaSuccess || e2 != cudaSuccess) { drop_graph(s); return cuda_fail(s, e != cudaSuccess ? e : e2, "homg_solve: capture(body)"); }
+    CU(s, census(body, s->solve_census));
+    s->solve_census[3] += 1;                                     // the WHILE node itself
     e = cudaGraphInstantiate(&s->solve_exec, s->solve_graph, 0);
     if (e != cudaSuccess) { drop_graph(s); return cuda_fail(s, e, "homg_solve: cudaGraphInstantiate"); }
     return HOMG_OK;
@@ -425,6 +449,20 @@ int homg_get_schedule(const homg_solver* s, int* lv, int* it, int cap) {
 }
 
 int homg_launches_per_cycle(const homg_solver* s) { return s ? s->launches_per_cycle : -1; }
+
+homg_status homg_graph_nodes(const homg_solver* s, int which, int* counts) {
+    if (!s || !counts) return HOMG_EINVAL;
+    for (int i = 0; i < 5; ++i) counts[i] = 0;
+    homg_solver* m = const_cast<homg_solver*>(s);
+    if (which == 0) {
+        if (!s->graph) return set_err(m, HOMG_ESTATE, "homg_graph_nodes before homg_cycle");
+        cudaError_t e = census(s->graph, counts);
+        return e == cudaSuccess ? HOMG_OK : cuda_fail(m, e, "census(cycle graph)");
+    }
+    if (!s->solve_graph) return set_err(m, HOMG_ESTATE, "homg_graph_nodes before homg_solve");
+    for (int i = 0; i < 5; ++i) counts[i] = s->solve_census[i];   // taken while the graph was built
+    return HOMG_OK;
+}
 
 double homg_bytes_per_cycle(const homg_solver* s, int level0_only) {
     if (!s) return -1.0;

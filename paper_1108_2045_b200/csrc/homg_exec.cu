@@ -360,8 +360,7 @@ void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, 
 template <class T, int ND, bool INTERP>
 void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
                      int a_assign, const T* d0, const T* v0, T* u) {
-    // (the S3e-bookkeeping form of levels >= 1 stays on homg_visit.cuh unless visit3 == 2: k_visit3<.., BOOK> needs
-    // more registers than 384 threads leave it)
+    // (visit3 == 1 keeps the S3e-bookkeeping form of levels >= 1 on homg_visit.cuh)
     if (ND == 3 && R.s->visit3 && (R.s->visit3 >= 2 || INTERP || !(a || o1 || o2))) {
         if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
         else if (ns == 3) launch_visit3<T, 3, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);

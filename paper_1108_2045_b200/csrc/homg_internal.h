@@ -83,7 +83,8 @@ struct homg_solver {
     bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
     int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
-    int visit3 = 1;                  // 3-D K_visit: homg_visit3.cuh (HOMG_VISIT3=0: the r01 kernel of homg_visit.cuh)
+    int visit3 = 2;                  // 3-D K_visit: 2 = homg_visit3.cuh for every form (default); 1 = only the level-0 / plain
+                                     // forms, bookkeeping visits on homg_visit.cuh; 0 = homg_visit.cuh (the r01 kernel) throughout
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create
     std::vector<int> sched_lv, sched_it;
@@ -106,6 +107,8 @@ struct homg_solver {
     cudaGraphExec_t graph_exec = nullptr;
     cudaGraph_t solve_graph = nullptr;   // homg_solve: S1, then a WHILE node whose body is one cycle (S2..S4, S1)
     cudaGraphExec_t solve_exec = nullptr;
+    cudaGraph_t solve_body = nullptr;    // the WHILE node's body (owned by solve_graph)
+    int solve_census[5] = {};            // kernel / memset / memcpy / conditional / other nodes of solve_graph + body
     void* solve_params = nullptr;        // device: SolveParams (tolerance^2, last history slot)
     bool have_rhs = false, have_coef = false;
     long cycles_issued = 0;

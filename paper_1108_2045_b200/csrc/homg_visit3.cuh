@@ -23,13 +23,14 @@
 
 namespace homg {
 
-// BOOK: the visit of a level >= 1 (S3e bookkeeping, three iterates stored) carries more live values per thread:
-// 320 threads (20 row pairs) at <= 204 registers instead of 384 at <= 168
+// BOOK: the visit of a level >= 1 (S3e bookkeeping, three iterates stored) carries more live values per thread
+// (226 registers): 256 threads (16 row pairs, tile 64 x 32) instead of 384 at <= 168.  (320 threads get no more
+// registers than 384: ptxas allots them per group of four warps.)
 template <class T, int NS, bool BOOK>
 struct Visit3Tile {
     static constexpr int ES = int(sizeof(T));
     static constexpr int VEC = 16 / ES;
-    static constexpr int PX = 16, TR = BOOK ? 20 : 24, NT = PX * TR;   // packs per row, row pairs, threads
+    static constexpr int PX = 16, TR = BOOK ? 16 : 24, NT = PX * TR;   // packs per row, row pairs, threads
     static constexpr int HX = (NS + VEC - 1) / VEC * VEC;      // x halo (nodes), pack granular
     static constexpr int HY = (NS + 1) / 2 * 2;                // y halo (rows), row-pair granular
     static constexpr int TXN = PX * VEC, PY = 2 * TR;          // tile in nodes
@@ -382,13 +383,15 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             dn = *reinterpret_cast<const Pack<T>*>(ctr + offE - RS);
             up = *reinterpret_cast<const Pack<T>*>(ctr + offO + RS);
         };
+        constexpr bool AHEAD = !BOOK;                              // (the bookkeeping form has no registers to spare)
         Pack<T> dnN, upN;
-        fetch(1, dnN, upN);
+        if (AHEAD) fetch(1, dnN, upN);
 #pragma unroll
         for (int s = 1; s <= NS; ++s) {
             // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
+            if (!AHEAD) fetch(s, dnN, upN);
             const Pack<T> dnE = dnN, upO = upN;
-            if (s < NS) fetch(s + 1, dnN, upN);
+            if (AHEAD && s < NS) fetch(s + 1, dnN, upN);
             const int z = z0 - s;
             const bool zin = STEADY || (z > 0 && z < NM - 1);
             Pack<T> out[2];

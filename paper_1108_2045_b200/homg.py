@@ -20,7 +20,7 @@ DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
 SYMBOLS = [
     "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
     "homg_set_coefficient", "homg_cycle", "homg_solve", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
-    "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_workspace_bytes_mixed", "homg_get_schedule", "homg_launches_per_cycle", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
+    "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_workspace_bytes_mixed", "homg_get_schedule", "homg_launches_per_cycle", "homg_graph_nodes", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
 ]
 
 
@@ -66,6 +66,7 @@ def lib():
         L.homg_residual_history.argtypes = [vp, C.POINTER(d), i, C.POINTER(i)]; L.homg_residual_history.restype = i
         L.homg_get_schedule.argtypes = [vp, C.POINTER(i), C.POINTER(i), i]; L.homg_get_schedule.restype = i
         L.homg_launches_per_cycle.argtypes = [vp]; L.homg_launches_per_cycle.restype = i
+        L.homg_graph_nodes.argtypes = [vp, i, C.POINTER(i)]; L.homg_graph_nodes.restype = i
         L.homg_bytes_per_cycle.argtypes = [vp, i]; L.homg_bytes_per_cycle.restype = d
         L.homg_profile_cycles.argtypes = [vp, i, C.POINTER(d), C.POINTER(i), C.POINTER(d), i]; L.homg_profile_cycles.restype = i
         L.homg_tag_name.argtypes = [i]; L.homg_tag_name.restype = C.c_char_p
@@ -210,6 +211,12 @@ class Solver:
 
     def launches_per_cycle(self):
         return int(lib().homg_launches_per_cycle(self.handle))
+
+    def graph_nodes(self, which=0):
+        """node census of the cycle graph (0) or of homg_solve's graph incl. its loop body (1)"""
+        c = (C.c_int * 5)()
+        self._ck(lib().homg_graph_nodes(self.handle, int(which), c))
+        return dict(zip(("kernel", "memset", "memcpy", "conditional", "other"), list(c)))
 
     def bytes_per_cycle(self, level0_only=False):
         return float(lib().homg_bytes_per_cycle(self.handle, 1 if level0_only else 0))

@@ -494,3 +494,82 @@ def test_mixed_precision_argument_checks():
     from paper_1108_2045_b200 import homg
     with pytest.raises(homg.HomgError):
         homg.Solver((33, 33, 33), 5, "poisson7", "f64", mixed=True, vcycle=(2, 1))
+
+
+# ---- compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md): the checks that remain ours ----
+@pytest.mark.parametrize("name,n,kw", [("cfg4", 65, {"tiled_min_nodes": 1}), ("cfg2", 33, {"tiled_min_nodes": 1}),
+                                       ("cfg3", 513, {"tiled_min_nodes": 1}), ("cfg5", 33, {"tiled_min_nodes": 1}),
+                                       ("cfg1", 129, {}), ("cfg4", 33, {"tiled_min_nodes": 1, "vcycle": True}),
+                                       ("cfg2", 33, {"tiled_min_nodes": 1, "mixed": True})])
+def test_no_write_outside_the_workspace(name, n, kw):
+    """the solver lives in a caller-owned workspace: 4 MiB of canaries on either side of it stay untouched by every
+    kernel family (ragged tiles, halo packs, TMA boxes, 16-byte row tails), and every array inside stays finite."""
+    import ctypes as C
+    torch = _torch()
+    from paper_1108_2045_b200 import homg
+    cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+    inp = I.make_inputs(cfg)
+    mixed = kw.pop("mixed", False)
+    vc = kw.pop("vcycle", False)
+    L = homg.lib()
+    dims = homg._dims(cfg.dims)
+    dt = "f64" if mixed else cfg.dtype
+    if mixed:
+        inp = {k: (None if v is None else v.astype(np.float64)) for k, v in inp.items()}
+        need = L.homg_workspace_bytes_mixed(len(cfg.dims), dims, cfg.levels, homg.STENCILS[cfg.stencil])
+    else:
+        need = L.homg_workspace_bytes(len(cfg.dims), dims, cfg.levels, homg.STENCILS[cfg.stencil], homg.DTYPES[dt])
+    pad = 4 << 20
+    buf = torch.full((need + 2 * pad,), 0xA5, dtype=torch.uint8, device="cuda")
+    o = homg.HomgOptions()
+    L.homg_default_options(C.byref(o))
+    o.omega, o.max_iters, o.tiled_min_nodes = cfg.omega, cfg.max_iters, int(kw.get("tiled_min_nodes", 0))
+    o.cuda_stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if vc:
+        o.cycle, o.v_eta1, o.v_eta2 = 1, 2, 1
+    if mixed:
+        o.mixed = 1
+    h = C.c_void_p(None)
+    assert (buf.data_ptr() + pad) % 256 == 0
+    rc = L.homg_create(C.byref(h), len(cfg.dims), dims, cfg.levels, homg.STENCILS[cfg.stencil], homg.DTYPES[dt],
+                       C.c_void_p(buf.data_ptr() + pad), need, C.byref(o))
+    assert rc == 0, L.homg_last_error(None)
+    dev = {k: (None if v is None else torch.from_numpy(v).cuda()) for k, v in inp.items()}
+    if dev["k"] is not None:
+        assert L.homg_set_coefficient(h, C.c_void_p(dev["k"].data_ptr()), 1) == 0
+    assert L.homg_set_rhs(h, C.c_void_p(dev["f"].data_ptr()), 1) == 0
+    assert L.homg_set_initial_guess(h, C.c_void_p(dev["u0"].data_ptr()), 1) == 0
+    assert L.homg_cycle(h, 3) == 0
+    if not vc and not mixed:
+        nd, rr = C.c_int(0), C.c_double(0)
+        assert L.homg_solve(h, 1e-30, 2, C.byref(nd), C.byref(rr)) == 0 and nd.value == 2
+    a, r = C.c_double(0), C.c_double(0)
+    assert L.homg_residual_norm(h, C.byref(a), C.byref(r)) == 0 and np.isfinite(a.value)
+    out = torch.empty(cfg.dims, dtype=dev["f"].dtype, device="cuda")
+    assert L.homg_get_solution(h, C.c_void_p(out.data_ptr()), 1) == 0
+    torch.cuda.synchronize()
+    assert bool((buf[:pad] == 0xA5).all()) and bool((buf[pad + need:] == 0xA5).all()), "a kernel wrote outside the workspace"
+    assert bool(torch.isfinite(out).all())
+    L.homg_destroy(h)
+
+
+def test_a_cycle_is_one_graph_of_kernels_and_memsets_only():
+    """"no host transfers inside a solve" (north_star): homg_cycle(n) = n replays of one CUDA graph, homg_solve = one
+    launch of a graph with a device-side WHILE node; neither graph holds a memcpy or host node."""
+    _torch()
+    from paper_1108_2045_b200 import homg
+    for name, n, kw in (("cfg4", 65, {"tiled_min_nodes": 200000}), ("cfg1", 129, {}), ("cfg5", 33, {})):
+        cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+        inp = I.make_inputs(cfg)
+        s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, cfg.dtype, omega=cfg.omega, max_iters=cfg.max_iters, **kw)
+        if inp["k"] is not None:
+            s.set_coefficient(inp["k"])
+        s.set_rhs(inp["f"])
+        s.cycle(1)
+        s.solve(1e-3, 5)
+        for which in (0, 1):
+            c = s.graph_nodes(which)
+            assert c["kernel"] == s.launches_per_cycle() + (2 if which == 1 else 0), (name, which, c)
+            assert c["memcpy"] == 0 and c["other"] == 0, (name, which, c)
+            assert c["conditional"] == which
+        s.destroy()
