@@ -19,6 +19,7 @@
 //   homg  alg=1 "H"          the same cycle carried on per-level arrays (what the GPU
 //                            implements); must equal L to rounding
 //   vcycle                   classic V(eta1,eta2) (L47)
+//   homg_p2                  section 3 (L77-85): the literal iteration on a 2-D grid of 2^k nodes per side
 //   dense_solve / assemble   dense LU of A u = f on tiny grids (fixed point of the cycle)
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): dense LU fixed point, Laplacian
@@ -692,6 +693,161 @@ int run_homg_mixed(int nd, const int64_t* dims, int levels, double h, const doub
     return 0;
 }
 
+
+// ---------------------------------------------------------------------------
+// Algorithm P — PAPER.md section 3 (L77-85), "Power of two size grids": the literal HOMG iteration on a 2-D grid
+// with N = 2^k nodes per side (N-1 intervals: not nestable).  Fig. 2 is not in the file; the reading is DESIGN.md R19:
+//   * the grid is divided into four subdomains of N/2 x N/2 nodes (L79, L83: "four subdomains with a power of two
+//     nodes per side"); per axis a node belongs to the LOW half (index < N/2) or the HIGH half;
+//   * the level-m coarse points of a subdomain are marked "relative to the corresponding external corner" (L83): per
+//     axis the low half's lattice is {i l}, the high half's {N-1 - i l}, l = 2^m, i = 0 .. N/(2l).  The last point,
+//     i = N/(2l), lies "just outside the corresponding subdomain" (L85) — the central points without which "some coarse
+//     modes, like the zero mode, can not be resolved" (`central` = 0 leaves them out: the pin that shows exactly that);
+//   * "We perform relaxations in all the marked points and interpolations on the rest of the fine grid" (L85): a marked
+//     interior node relaxes with the stride-l stencil of Eq. 3 IN THE FINE ARRAY (its neighbours at distance l need not be
+//     marked; an index outside the grid counts as the Dirichlet value 0); its source is the weighted-average restriction
+//     P_m r on ITS lattice: each of the 2 x 2 anchor combinations is a nested lattice of the (N+1)-node grid obtained by
+//     adding one ghost row / column (value 0) beyond the side opposite to the anchor, so "nested partial reductions"
+//     (L73) apply to each unchanged;
+//   * every other node adds the bilinear interpolation of the previous-iteration variations of the marked nodes of ITS
+//     OWN subdomain's lattice: "The interpolations make use only of points in the same subdomain" (L85).
+// Everything else (schedule, restart, one-iteration delay, Eq. 3 arithmetic) is Algorithm L's.
+// ---------------------------------------------------------------------------
+struct P2Lattice {
+    int64_t N, l;
+    bool central;
+    int64_t last() const { return central ? N / 2 : N / 2 - 1; }      // largest distance from the anchor that is marked
+    // is coordinate x on the low- / high-anchored lattice?  *anchor = 0 (low) or 1 (high); level 0: every x, anchor 0
+    bool on(int64_t x, int* anchor) const {
+        if (x % l == 0 && x <= last()) { *anchor = 0; return true; }
+        const int64_t t = N - 1 - x;
+        if (t % l == 0 && t <= last()) { *anchor = 1; return true; }
+        return false;
+    }
+};
+
+// E[ay][ax][m]: nested full weighting of the residual on the lattice anchored at corner (ay, ax); arrays of
+// (N / 2^m + 1)^2 entries indexed FROM THE ANCHOR, the last row / column being the ghost (0)
+template <class T>
+void p2_restrict_all(int64_t N, int levels, const T* r, std::vector<std::vector<T>> E[2][2]) {
+    for (int ay = 0; ay < 2; ++ay)
+        for (int ax = 0; ax < 2; ++ax) {
+            auto& H = E[ay][ax];
+            H.assign(levels, std::vector<T>());
+            H[0].assign(size_t((N + 1) * (N + 1)), T(0));
+            for (int64_t i = 0; i < N; ++i)
+                for (int64_t j = 0; j < N; ++j)
+                    H[0][size_t(i * (N + 1) + j)] = r[(ay ? N - 1 - i : i) * N + (ax ? N - 1 - j : j)];
+            int64_t n = N + 1;
+            for (int m = 1; m < levels; ++m) {
+                int64_t d[2] = {n, n};
+                Grid F = make_grid(2, d);
+                n = (n - 1) / 2 + 1;
+                H[m].assign(size_t(n * n), T(0));
+                restrict_fw(F, H[m - 1].data(), H[m].data());
+            }
+        }
+}
+
+template <class T>
+void iteration_P(int64_t N, int m, double h, double omega, bool central, std::vector<std::vector<T>> E[2][2],
+                 std::vector<T>& cur, std::vector<T>& prev, std::vector<T>& nxt, std::vector<T>& var) {
+    const int64_t l = int64_t(1) << m;
+    const P2Lattice Lt{N, l, central};
+    const double hm = double(l) * h;
+    const T h2 = T(hm * hm), wp = T(omega / 4.0);
+    for (int64_t i = 0; i < N * N; ++i) var[size_t(i)] = cur[size_t(i)] - prev[size_t(i)];
+    auto at = [&](int64_t y, int64_t x) -> T { return (y < 0 || y >= N || x < 0 || x >= N) ? T(0) : cur[size_t(y * N + x)]; };
+    for (int64_t y = 0; y < N; ++y)
+        for (int64_t x = 0; x < N; ++x) {
+            const size_t c = size_t(y * N + x);
+            if (y == 0 || y == N - 1 || x == 0 || x == N - 1) { nxt[c] = 0; continue; }
+            int ay = 0, ax = 0;
+            if (Lt.on(y, &ay) && Lt.on(x, &ax)) {
+                // relaxation, Eq. 3 (same three fused multiply-adds as jacobi_node)
+                const int64_t nl = N / l + 1;
+                const int64_t iy = (ay ? N - 1 - y : y) / l, ix = (ax ? N - 1 - x : x) / l;
+                const T g = E[ay][ax][m][size_t(iy * nl + ix)];
+                T s = 0;
+                s += at(y - l, x) + at(y + l, x);
+                s += at(y, x - l) + at(y, x + l);
+                T t = std::fma(-T(4), cur[c], s);
+                t = std::fma(h2, g, t);
+                nxt[c] = std::fma(wp, t, cur[c]);
+                ++g_relax_updates;
+            } else {
+                // interpolation of the previous variations on the lattice of the node's own subdomain
+                int64_t c0[2], c1[2];
+                T wl[2], wh[2];
+                const int64_t pp[2] = {y, x};
+                for (int a = 0; a < 2; ++a) {
+                    const bool high = pp[a] >= N / 2;
+                    const int64_t t = high ? N - 1 - pp[a] : pp[a];
+                    const int64_t i0 = t / l;
+                    wh[a] = T(double(t - i0 * l) / double(l));
+                    wl[a] = T(1) - wh[a];
+                    c0[a] = high ? N - 1 - i0 * l : i0 * l;
+                    c1[a] = high ? N - 1 - (i0 + 1) * l : (i0 + 1) * l;
+                }
+                T acc = 0;
+                for (int cy = 0; cy < 2; ++cy)
+                    for (int cx = 0; cx < 2; ++cx) {
+                        const T wy = cy ? wh[0] : wl[0], wx = cx ? wh[1] : wl[1];
+                        if (wy == T(0) || wx == T(0)) continue;
+                        const int64_t qy = cy ? c1[0] : c0[0], qx = cx ? c1[1] : c0[1];
+                        acc += (wy * wx) * var[size_t(qy * N + qx)];
+                    }
+                nxt[c] = cur[c] + acc;
+                ++g_move_updates;
+            }
+        }
+    prev.swap(cur);
+    cur.swap(nxt);
+}
+
+template <class T>
+double cycle_P(int64_t N, int levels, double h, double omega, bool central, const int* slv, const int* sit, int slen,
+               const T* f, T* u, long max_iters, T* cur_out) {
+    int64_t d[2] = {N, N};
+    Grid F = make_grid(2, d);
+    std::vector<T> r(size_t(N * N), T(0));
+    double n2 = residual(F, h, (const T*)nullptr, u, f, r.data());
+    std::vector<std::vector<T>> E[2][2];
+    p2_restrict_all(N, levels, r.data(), E);
+    std::vector<T> cur(size_t(N * N), T(0)), prev(size_t(N * N), T(0)), nxt(size_t(N * N), T(0)), var(size_t(N * N), T(0));
+    long done = 0;
+    for (int s = 0; s < slen && (max_iters < 0 || done < max_iters); ++s)
+        for (int it = 0; it < sit[s] && (max_iters < 0 || done < max_iters); ++it, ++done)
+            iteration_P(N, slv[s], h, omega, central, E, cur, prev, nxt, var);
+    if (cur_out) std::memcpy(cur_out, cur.data(), sizeof(T) * size_t(N * N));
+    for (int64_t i = 0; i < N * N; ++i) u[i] += cur[size_t(i)];
+    return std::sqrt(n2);
+}
+
+inline bool p2_valid(int64_t N, int levels) {
+    if (N < 8 || (N & (N - 1)) != 0 || levels < 1) return false;
+    return (int64_t(1) << (levels - 1)) <= N / 2;           // coarsest lattice: {anchor, central point} per half
+}
+
+template <class T>
+int run_homg_p2(int64_t N, int levels, double h, double omega, int central, const int* slv, const int* sit, int slen,
+                const void* f_, void* u_, int ncycles, void* hist_, double* norms) {
+    if (!p2_valid(N, levels)) return 1;
+    for (int s = 0; s < slen; ++s) if (slv[s] < 0 || slv[s] >= levels || sit[s] < 1) return 2;
+    const T* f = (const T*)f_;
+    T* u = (T*)u_;
+    T* hist = (T*)hist_;
+    for (int c = 0; c < ncycles; ++c) {
+        double n = cycle_P<T>(N, levels, h, omega, central != 0, slv, sit, slen, f, u, -1, nullptr);
+        if (norms) norms[c] = n;
+        if (hist) std::memcpy(hist + size_t(c) * size_t(N * N), u, sizeof(T) * size_t(N * N));
+    }
+    int64_t d[2] = {N, N};
+    Grid F = make_grid(2, d);
+    if (norms) norms[ncycles] = std::sqrt(residual(F, h, (const T*)nullptr, u, f, (T*)nullptr));
+    return 0;
+}
+
 }  // namespace
 
 #define DISPATCH(dtype, CALL32, CALL64) ((dtype) == 4 ? (CALL32) : (dtype) == 8 ? (CALL64) : -1)
@@ -804,6 +960,53 @@ int64_t orc_assemble(int nd, const int64_t* dims, double h, const double* k, dou
     assemble<double>(G, h, k, M);
     std::memcpy(A, M.data(), sizeof(double) * N * N);
     return N;
+}
+
+// ---- Algorithm P (section 3, power-of-two grids; R19) ----
+// ncycles outer cycles on an N x N grid, N = 2^k, levels <= k.  central = 0 leaves out the central points (ablation pin).
+int orc_homg_p2(int dtype, int64_t N, int levels, double h, double omega, int central, const int* slv, const int* sit,
+                int slen, const void* f, void* u, int ncycles, void* u_hist, double* norms) {
+    if (dtype == 4) return run_homg_p2<float>(N, levels, h, omega, central, slv, sit, slen, f, u, ncycles, u_hist, norms);
+    if (dtype == 8) return run_homg_p2<double>(N, levels, h, omega, central, slv, sit, slen, f, u, ncycles, u_hist, norms);
+    return -1;
+}
+// the correction array after the first `niters` whole-grid iterations of one cycle (u is not modified)
+int orc_homg_p2_partial(int64_t N, int levels, double h, double omega, int central, const int* slv, const int* sit, int slen,
+                        const double* f, const double* u, long niters, double* cur_out) {
+    if (!p2_valid(N, levels)) return 1;
+    std::vector<double> uu(u, u + N * N);
+    cycle_P<double>(N, levels, h, omega, central != 0, slv, sit, slen, f, uu.data(), niters, cur_out);
+    return 0;
+}
+// mask[y*N+x] = 1 where node (y, x) is marked at level m (boundary nodes included)
+int orc_p2_marked(int64_t N, int m, int central, unsigned char* mask) {
+    P2Lattice Lt{N, int64_t(1) << m, central != 0};
+    for (int64_t y = 0; y < N; ++y)
+        for (int64_t x = 0; x < N; ++x) {
+            int a;
+            mask[y * N + x] = (Lt.on(y, &a) && Lt.on(x, &a)) ? 1 : 0;
+        }
+    return 0;
+}
+// one iteration at level m with source 0 from (cur, prev): out = next iterate.  With cur = d, prev = 0 the non-marked
+// nodes of `out` hold d + (interpolant of d on their subdomain's lattice): the interpolation operator alone.
+int orc_p2_iteration(int64_t N, int levels, int m, double h, double omega, int central, const double* r, const double* cur,
+                     const double* prev, double* out) {
+    if (!p2_valid(N, levels) || m < 0 || m >= levels) return 1;
+    std::vector<std::vector<double>> E[2][2];
+    p2_restrict_all<double>(N, levels, r, E);
+    std::vector<double> c(cur, cur + N * N), p(prev, prev + N * N), n(size_t(N * N), 0.0), v(size_t(N * N), 0.0);
+    iteration_P<double>(N, m, h, omega, central != 0, E, c, p, n, v);
+    std::memcpy(out, c.data(), sizeof(double) * size_t(N * N));
+    return 0;
+}
+// the restricted source of level m on the lattice anchored at (ay, ax): (N/2^m + 1)^2 entries indexed from the anchor
+int orc_p2_restrict(int64_t N, int levels, int m, int ay, int ax, const double* r, double* out) {
+    if (!p2_valid(N, levels) || m < 0 || m >= levels) return 1;
+    std::vector<std::vector<double>> E[2][2];
+    p2_restrict_all<double>(N, levels, r, E);
+    std::memcpy(out, E[ay][ax][m].data(), sizeof(double) * E[ay][ax][m].size());
+    return 0;
 }
 
 void orc_counters(unsigned long long* relax, unsigned long long* moves, int reset) {

@@ -175,3 +175,54 @@ def counters(reset=False):
     r = C.c_ulonglong(0); m = C.c_ulonglong(0)
     lib().orc_counters(C.byref(r), C.byref(m), int(reset))
     return r.value, m.value
+
+
+# ---- Algorithm P: PAPER.md section 3, power-of-two grids (2-D; R19) ----
+def homg_p2(f, u0, levels, omega, sched, ncycles, h=None, central=True, keep_history=True):
+    f = _c(f); u = np.array(u0, dtype=f.dtype, order="C", copy=True)
+    N = f.shape[0]
+    assert f.ndim == 2 and f.shape == (N, N)
+    hist = np.empty((ncycles, N, N), dtype=f.dtype) if keep_history else None
+    norms = np.zeros(ncycles + 1, dtype=np.float64)
+    lv, it, n = _sched_arrays(sched)
+    rc = lib().orc_homg_p2(_dt(f), C.c_int64(N), levels, C.c_double(h or default_h(f.shape)), C.c_double(omega),
+                           int(bool(central)), lv, it, n, _p(f), _p(u), ncycles, _p(hist),
+                           norms.ctypes.data_as(C.POINTER(C.c_double)))
+    assert rc == 0, rc
+    return u, hist, norms
+
+
+def homg_p2_partial(f, u0, levels, omega, sched, niters, h=None, central=True):
+    f = _c(f, np.float64); u = _c(u0, np.float64)
+    N = f.shape[0]
+    cur = np.empty_like(f)
+    lv, it, n = _sched_arrays(sched)
+    rc = lib().orc_homg_p2_partial(C.c_int64(N), levels, C.c_double(h or default_h(f.shape)), C.c_double(omega),
+                                   int(bool(central)), lv, it, n, _p(f), _p(u), C.c_long(niters), _p(cur))
+    assert rc == 0, rc
+    return cur
+
+
+def p2_marked(N, m, central=True):
+    mask = np.zeros((N, N), dtype=np.uint8)
+    assert lib().orc_p2_marked(C.c_int64(N), m, int(bool(central)), mask.ctypes.data_as(C.c_void_p)) == 0
+    return mask.astype(bool)
+
+
+def p2_iteration(r, cur, prev, levels, m, omega, h=None, central=True):
+    r = _c(r, np.float64); cur = _c(cur, np.float64); prev = _c(prev, np.float64)
+    N = r.shape[0]
+    out = np.empty_like(r)
+    rc = lib().orc_p2_iteration(C.c_int64(N), levels, m, C.c_double(h or default_h(r.shape)), C.c_double(omega),
+                                int(bool(central)), _p(r), _p(cur), _p(prev), _p(out))
+    assert rc == 0, rc
+    return out
+
+
+def p2_restrict(r, levels, m, ay, ax):
+    r = _c(r, np.float64)
+    N = r.shape[0]
+    n = N // (1 << m) + 1
+    out = np.empty((n, n), dtype=np.float64)
+    assert lib().orc_p2_restrict(C.c_int64(N), levels, m, ay, ax, _p(r), _p(out)) == 0
+    return out

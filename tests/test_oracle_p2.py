@@ -1,0 +1,250 @@
+"""Pins for the oracle's Algorithm P — PAPER.md section 3 (L77-85), HOMG on 2-D grids with a power-of-two number of
+nodes per side (R19; Fig. 2 is not in the file).  Against what the paper says and the mathematics fixes:
+
+  P12a marked sets: four lattices, each relative to its external corner; the points just outside a subdomain (L83-85)
+  P12b interpolation uses the node's own subdomain only and is exact on bilinear functions inside it (L85)
+  P12c restriction on every lattice = the composite full-weighting (hat) weights; constants -> constants (L73)
+  P12d relaxation at a marked node = Eq. 3 with stride l in the fine array (L65), out-of-grid neighbours = 0
+  P12e fixed point = the dense LU solution of A u = f on the N x N grid; O(h^2) on Eq. 5-6
+  P12f the zero mode: with the central points the cycle contracts at a grid-independent rate; without them it does
+       not ("some coarse modes, like the zero mode, can not be resolved", L85)
+  P12g first iterations (L113): only the middle points move in iteration 1; iteration 2 builds a pyramid
+"""
+import numpy as np
+import pytest
+
+from paper_1108_2045_b200 import inputs as I
+
+
+def sine_f(N):
+    y, x = np.meshgrid(np.arange(N) / (N - 1), np.arange(N) / (N - 1), indexing="ij")
+    f = 2 * np.pi ** 2 * np.sin(np.pi * x) * np.sin(np.pi * y)
+    f[0] = f[-1] = 0
+    f[:, 0] = f[:, -1] = 0
+    return f
+
+
+def test_P12a_marked_sets(orc):
+    # N = 16, l = 4: low lattice {0, 4, 8}, high lattice {15, 11, 7}: 8 = N/2 and 7 = N/2 - 1 are the points "just
+    # outside the corresponding subdomain" (the low half is 0..7, the high half 8..15)
+    m = orc.p2_marked(16, 2)
+    coords = sorted({0, 4, 8, 15, 11, 7})
+    want = np.zeros((16, 16), bool)
+    want[np.ix_(coords, coords)] = True
+    assert np.array_equal(m, want)
+    # without the central points
+    m0 = orc.p2_marked(16, 2, central=False)
+    c0 = sorted({0, 4, 15, 11})
+    w0 = np.zeros((16, 16), bool)
+    w0[np.ix_(c0, c0)] = True
+    assert np.array_equal(m0, w0)
+    # level 0: every node; coarsest level (l = N/2): the corners and the central 2 x 2 block and their products
+    assert orc.p2_marked(16, 0).all()
+    mc = orc.p2_marked(16, 3)
+    cc = [0, 7, 8, 15]
+    wc = np.zeros((16, 16), bool)
+    wc[np.ix_(cc, cc)] = True
+    assert np.array_equal(mc, wc)
+    # every level's marked set contains the next coarser one (nested inside each lattice), and is symmetric
+    for N in (16, 64):
+        k = int(np.log2(N))
+        for lv in range(k - 1):
+            a, b = orc.p2_marked(N, lv), orc.p2_marked(N, lv + 1)
+            assert not (b & ~a).any()
+            assert np.array_equal(a, a[::-1]) and np.array_equal(a, a.T)
+            per_axis = 2 * (N // 2 // (1 << lv) + 1) if lv > 0 else N
+            assert a.sum() == per_axis ** 2
+
+
+@pytest.mark.parametrize("N,m", [(16, 1), (16, 2), (32, 3), (64, 2), (64, 5)])
+def test_P12b_interpolation_stays_in_the_subdomain_and_is_bilinear_exact(orc, N, m):
+    k = int(np.log2(N))
+    mk = orc.p2_marked(N, m)
+    zero = np.zeros((N, N))
+    y, x = np.meshgrid(np.arange(N, dtype=float), np.arange(N, dtype=float), indexing="ij")
+    inner = np.zeros((N, N), bool)
+    inner[1:-1, 1:-1] = True
+    rest = ~mk & inner
+    # a different bilinear function in every subdomain: each is reproduced exactly where the subdomain interpolates
+    rng = np.random.default_rng(4)
+    d = np.zeros((N, N))
+    want = np.zeros((N, N))
+    for qy in (0, 1):
+        for qx in (0, 1):
+            a, b, c, e = rng.standard_normal(4)
+            fn = a + b * x + c * y + e * x * y
+            ys = slice(0, N // 2) if qy == 0 else slice(N // 2, N)
+            xs = slice(0, N // 2) if qx == 0 else slice(N // 2, N)
+            want[ys, xs] = fn[ys, xs]
+            # the lattice of this subdomain: its marked coordinates reach one point beyond the half
+            l = 1 << m
+            cy = [i * l for i in range(N // 2 // l + 1)] if qy == 0 else [N - 1 - i * l for i in range(N // 2 // l + 1)]
+            cx = [i * l for i in range(N // 2 // l + 1)] if qx == 0 else [N - 1 - i * l for i in range(N // 2 // l + 1)]
+            d[np.ix_(cy, cx)] = fn[np.ix_(cy, cx)]          # (the lattices are disjoint for l >= 2: N - 1 is odd)
+    out = orc.p2_iteration(zero, d, zero, k, m, 0.8)         # cur = d, prev = 0, no source
+    assert np.allclose(out[rest], (d + want)[rest], rtol=0, atol=1e-12 * np.abs(want).max())
+    # constants: weights sum to one
+    out = orc.p2_iteration(zero, np.where(mk, 3.0, 0.0), zero, k, m, 0.8)
+    assert np.allclose(out[rest], 3.0, atol=1e-14)
+    # no cross-domain data: a variation on the OTHER subdomains' lattices only leaves this subdomain's nodes alone
+    l = 1 << m
+    lowc = [i * l for i in range(N // 2 // l + 1)]
+    other = mk.copy()
+    other[np.ix_(lowc, lowc)] = False                         # everything except the (low, low) lattice
+    out = orc.p2_iteration(zero, np.where(other, 1.0, 0.0), zero, k, m, 0.8)
+    ll = np.zeros((N, N), bool)
+    ll[: N // 2, : N // 2] = True
+    assert np.all(out[rest & ll] == 0)
+
+
+@pytest.mark.parametrize("N,m", [(16, 1), (32, 2), (64, 3)])
+def test_P12c_restriction_is_the_composite_full_weighting_on_every_lattice(orc, N, m):
+    k = int(np.log2(N))
+    l = 1 << m
+    rng = np.random.default_rng(6)
+    r = np.zeros((N, N))
+    r[1:-1, 1:-1] = rng.standard_normal((N - 2, N - 2))
+    hat = np.array([(l - abs(d)) / l ** 2 for d in range(-l + 1, l)])      # m-fold composition of [1 2 1]/4 at strides 1, 2, ..
+    for ay in (0, 1):
+        for ax in (0, 1):
+            g = orc.p2_restrict(r, k, m, ay, ax)
+            assert g.shape == (N // l + 1, N // l + 1)
+            rr = r[::-1] if ay else r
+            rr = rr[:, ::-1] if ax else rr
+            ext = np.zeros((N + 1 + 2 * l, N + 1 + 2 * l))
+            ext[l:l + N, l:l + N] = rr
+            # away from the faces, where nested full weighting truncates (its coarse boundary entries are 0)
+            for i in range(2, N // l - 1):
+                for j in range(2, N // l - 1):
+                    win = ext[l + i * l - l + 1:l + i * l + l, l + j * l - l + 1:l + j * l + l]
+                    assert abs(g[i, j] - hat @ win @ hat) < 1e-13
+            assert np.all(g[0] == 0) and np.all(g[-1] == 0) and np.all(g[:, 0] == 0) and np.all(g[:, -1] == 0)
+    ones = np.zeros((N, N))
+    ones[1:-1, 1:-1] = 1.0
+    g = orc.p2_restrict(ones, k, m, 1, 0)
+    assert np.allclose(g[2:-2, 2:-2], 1.0, atol=1e-14)
+
+
+def test_P12d_relaxation_at_marked_nodes_is_eq3_with_stride_l(orc):
+    N, k, m, omega, h = 32, 5, 2, 0.8, 1.0 / 31
+    l = 1 << m
+    rng = np.random.default_rng(8)
+    cur = np.zeros((N, N))
+    cur[1:-1, 1:-1] = rng.standard_normal((N - 2, N - 2))
+    r = np.zeros((N, N))
+    r[1:-1, 1:-1] = rng.standard_normal((N - 2, N - 2))
+    out = orc.p2_iteration(r, cur, cur, k, m, omega, h=h)       # prev = cur: the interpolating nodes do not move
+    mk = orc.p2_marked(N, m)
+    inner = np.zeros((N, N), bool)
+    inner[1:-1, 1:-1] = True
+    assert np.array_equal(out[~mk & inner], cur[~mk & inner])
+    pad = np.zeros((N + 2 * l, N + 2 * l))
+    pad[l:l + N, l:l + N] = cur
+    lowc = [i * l for i in range(N // 2 // l + 1)]
+    highc = [N - 1 - i * l for i in range(N // 2 // l + 1)]
+    g = {(ay, ax): orc.p2_restrict(r, k, m, ay, ax) for ay in (0, 1) for ax in (0, 1)}
+    hl2 = (l * h) ** 2
+    checked = 0
+    for y in range(1, N - 1):
+        for x in range(1, N - 1):
+            if not mk[y, x]:
+                continue
+            ay, ax = (0 if y in lowc else 1), (0 if x in lowc else 1)
+            src = g[(ay, ax)][(N - 1 - y if ay else y) // l, (N - 1 - x if ax else x) // l]
+            s = pad[y, x + l] + pad[y + 2 * l, x + l] + pad[y + l, x] + pad[y + l, x + 2 * l]
+            want = cur[y, x] + omega / 4 * ((s - 4 * cur[y, x]) + hl2 * src)     # PAPER.md L65 Eq. 3, sign of DESIGN.md R1
+            assert abs(out[y, x] - want) < 1e-13 * max(1.0, abs(want))
+            checked += 1
+    assert checked == (2 * (N // 2 // l + 1) - 2) ** 2
+    assert not out[0].any() and not out[-1].any() and not out[:, 0].any() and not out[:, -1].any()
+
+
+@pytest.mark.parametrize("N", [8, 16])
+def test_P12e_fixed_point_is_the_dense_lu_solution(orc, N):
+    k = int(np.log2(N))
+    rng = np.random.default_rng(10)
+    f = np.zeros((N, N))
+    f[1:-1, 1:-1] = rng.standard_normal((N - 2, N - 2))
+    h = 1.0 / (N - 1)
+    ulu = orc.dense_solve(f, h=h)
+    u, _, norms = orc.homg_p2(f, np.zeros_like(f), k, 0.8, orc.schedule(0, k, 4), 60, h=h, keep_history=False)
+    assert np.max(np.abs(u - ulu)) <= 1e-12 * np.max(np.abs(ulu))
+    assert norms[-1] <= 1e-12 * norms[0]
+    # zero residual: the cycle returns a zero correction
+    f2 = orc.apply_A(ulu, h=h)
+    u2, _, n2 = orc.homg_p2(f2, ulu, k, 0.8, orc.schedule(0, k, 4), 1, h=h, keep_history=False)
+    assert np.max(np.abs(u2 - ulu)) <= 1e-13 * np.max(np.abs(ulu))
+
+
+def test_P12e_second_order_on_the_papers_polynomial(orc):
+    """PAPER.md Eq. 5-6 on 2^k grids: the converged solution approaches u = -x^2 y^2 (1-x^2)(1-y^2) as h^2."""
+    errs = []
+    for N in (16, 32, 64):
+        k = int(np.log2(N))
+        f, uex = I.paper_polynomial((N, N))
+        u, _, norms = orc.homg_p2(f, np.zeros_like(f), k, 0.8, orc.schedule(0, k, 4), 30, keep_history=False)
+        assert norms[-1] <= 1e-10 * norms[0]
+        errs.append(np.max(np.abs(u - uex)))
+    h = [1.0 / 15, 1.0 / 31, 1.0 / 63]
+    for a in (0, 1):
+        rate = np.log(errs[a] / errs[a + 1]) / np.log(h[a] / h[a + 1])
+        assert 1.8 < rate < 2.2, (errs, rate)
+
+
+def test_P12f_the_central_points_resolve_the_zero_mode(orc):
+    """"The coarse subsets need to include central points, if not, some coarse modes, like the zero mode,
+    can not be resolved."  With them the asymptotic factor per cycle is grid independent; without them it tends to 1."""
+    with_c, without = [], []
+    for N in (16, 32, 64, 128):
+        k = int(np.log2(N))
+        f = sine_f(N)
+        for central, acc in ((True, with_c), (False, without)):
+            _, _, n = orc.homg_p2(f, np.zeros_like(f), k, 0.8, orc.schedule(0, k, 4), 8, central=central, keep_history=False)
+            acc.append(n[8] / n[7])
+    assert max(with_c) < 0.30 and max(with_c) - min(with_c) < 0.12, with_c
+    assert min(without) > 0.6, without
+    assert without == sorted(without) and without[-1] > 0.9, without        # worse with every refinement
+
+
+def test_P12g_first_iterations_spike_then_pyramid(orc):
+    """PAPER.md L113, for its 128^2 grid: "During the first iteration we see a spike because only the middle points
+    perform a relaxation and the interpolations have null sources. ... The second iteration shows that the relaxations
+    have stalled while the interpolations form the zero mode approximation with pyramid shape." """
+    N, k = 128, 7
+    f = sine_f(N)
+    sched = orc.schedule(0, k, 2)
+    zero = np.zeros_like(f)
+    h = 1.0 / (N - 1)
+    # omega = 1: the four middle points are decoupled at l = N/2 (their stride-l neighbours are the boundary / outside)
+    c1 = orc.homg_p2_partial(f, zero, k, 1.0, sched, 1)
+    mid = [N // 2 - 1, N // 2]
+    mask = np.zeros((N, N), bool)
+    mask[np.ix_(mid, mid)] = True
+    assert np.all(c1[~mask] == 0) and np.all(c1[mask] > 0)                  # "only the middle points"
+    g = orc.p2_restrict(f, k, k - 1, 0, 0)[1, 1]
+    assert abs(c1[N // 2, N // 2] - ((N // 2) * h) ** 2 * g / 4) < 1e-14     # omega h_M^2 g / 4 (pin P6's spike)
+    c2 = orc.homg_p2_partial(f, zero, k, 1.0, sched, 2)
+    assert np.allclose(c2[mask], c1[mask], rtol=1e-14)                      # "the relaxations have stalled" (omega = 1)
+    # the pyramid: inside every subdomain the bilinear function through 0 on the two outer faces and the spike value at
+    # its central point; monotone towards the middle
+    apex = c1[N // 2, N // 2]
+    for y in range(1, N // 2 - 1):
+        for x in range(1, N // 2 - 1):
+            assert abs(c2[y, x] - apex * (y / (N / 2)) * (x / (N / 2))) < 1e-13 * apex
+    row = c2[N // 4, : N // 2]
+    assert np.all(np.diff(row[1:]) > 0)
+    assert np.allclose(c2, c2[::-1], atol=1e-15) and np.allclose(c2, c2.T, atol=1e-15)
+
+
+def test_float32_and_argument_checks(orc):
+    N, k = 32, 5
+    f = sine_f(N)
+    sched = orc.schedule(0, k, 4)
+    u64, _, n64 = orc.homg_p2(f, np.zeros_like(f), k, 0.8, sched, 3, keep_history=False)
+    u32, _, n32 = orc.homg_p2(f.astype(np.float32), np.zeros((N, N), np.float32), k, 0.8, sched, 3, keep_history=False)
+    assert u32.dtype == np.float32
+    assert np.max(np.abs(u32 - u64)) <= 2e-5 * np.max(np.abs(u64))
+    with pytest.raises(AssertionError):
+        orc.homg_p2(np.zeros((33, 33)), np.zeros((33, 33)), 5, 0.8, sched, 1)          # not a power of two
+    with pytest.raises(AssertionError):
+        orc.homg_p2(f, np.zeros_like(f), 6, 0.8, orc.schedule(0, 6, 4), 1)              # l = 32 > N/2
