@@ -14,7 +14,7 @@
  * Conventions
  *   - dims[a] = nodes per axis INCLUDING the two Dirichlet boundary nodes, dims[0]
  *     slowest (C order).  ndim = 2: (ny, nx); ndim = 3: (nz, ny, nx).
- *   - every dims[a] must equal c_a * 2^(levels-1) + 1 with c_a >= 2.
+ *   - every dims[a] must equal c_a * 2^(levels-1) + 1 with c_a >= 2 (HOMG_POISSON5_POW2: see there).
  *   - level m = 0 is the finest; level m has (dims[a]-1)/2^m + 1 nodes per axis and
  *     mesh width h_m = 2^m h.
  *   - user arrays (f, u0, k, solution) are DENSE C-order arrays of prod(dims) scalars
@@ -60,8 +60,14 @@ typedef enum { HOMG_F32 = 4, HOMG_F64 = 8 } homg_dtype;
 typedef enum {
     HOMG_POISSON5 = 0,  /* 2-D, 5-point  -lap                     (Eq.3) */
     HOMG_POISSON7 = 1,  /* 3-D, 7-point  -lap                     (R10)        */
-    HOMG_DIFFUSION7 = 2 /* 3-D, 7-point  -div(k grad), nodal k,
+    HOMG_DIFFUSION7 = 2, /* 3-D, 7-point  -div(k grad), nodal k,
                            harmonic-mean faces, rediscretised per level (R11)  */
+    HOMG_POISSON5_POW2 = 3 /* 2-D, 5-point -lap on a grid with a POWER OF TWO number of nodes per side
+                           (section 3; R19): dims = (N, N), N = 2^k >= 8,
+                           levels <= k.  Four subdomains, coarse points relative to each external corner
+                           with the central points just outside every subdomain, same-subdomain
+                           interpolation.  Runs the paper's whole-grid iteration (one launch per
+                           iteration over the fine grid, as HOMG_CYCLE_LITERAL), whatever `cycle` says */
 } homg_stencil;
 
 /* MFMG schedule kinds (Fig.1 is missing — DESIGN.md R3).

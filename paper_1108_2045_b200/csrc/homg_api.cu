@@ -163,6 +163,7 @@ homg_status homg_create(homg_solver** out, int ndim, const int64_t* dims, int le
     if (!opt || !opt->mixed) return create_one(out, ndim, dims, levels, st, dt, ws, ws_bytes, opt);
     // mixed precision: an fp64 one-level outer problem (u, f, r) + the fp32 hierarchy of the correction cycle
     if (dt != HOMG_F64) return set_err(nullptr, HOMG_EINVAL, "mixed precision: dtype must be HOMG_F64 (u, f, k are fp64)");
+    if (st == HOMG_POISSON5_POW2) return set_err(nullptr, HOMG_EINVAL, "mixed precision is not available for HOMG_POISSON5_POW2");
     if (opt->cycle != HOMG_CYCLE_MFMG) return set_err(nullptr, HOMG_EINVAL, "mixed precision runs the MFMG cycle only");
     homg_options o = *opt;
     o.mixed = 0;
@@ -221,7 +222,10 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_VISIT3")) s->visit3 = std::atoi(ev);
     s->vcycle = o.cycle == HOMG_CYCLE_V;
-    s->literal = o.cycle == HOMG_CYCLE_LITERAL;
+    s->pow2 = P.pow2;
+    s->literal = o.cycle == HOMG_CYCLE_LITERAL || P.pow2;
+    if (P.pow2 && o.cycle == HOMG_CYCLE_V) { delete s; return set_err(nullptr, HOMG_EINVAL, "HOMG_POISSON5_POW2 runs the whole-grid HOMG iteration, not the V cycle"); }
+    if (P.pow2) s->vcycle = false;
     s->v_eta1 = o.v_eta1 >= 0 ? o.v_eta1 : 2;
     s->v_eta2 = o.v_eta2 >= 0 ? o.v_eta2 : 1;
     s->stream = static_cast<cudaStream_t>(o.cuda_stream);
@@ -252,6 +256,12 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
         L.h = s->h * double(1LL << m);
         size_t ab = L.n_alloc * es;
         L.nrot = (m == 0) ? 3 : kNumRot;
+        if (P.pow2 && m >= 1) {                    // PAPER.md section 3: only the restricted sources live on levels >= 1
+            for (int a = 0; a < 4; ++a) s->p2src[a][m] = take(ab);
+            L.gsrc = s->p2src[0][m];
+            L.nrot = 0;
+            continue;
+        }
         if (m == 0) { s->u = take(ab); s->f = take(ab); }
         L.gsrc = take(ab);
         for (int b = 0; b < L.nrot; ++b) L.rot[b] = take(ab);

@@ -16,6 +16,7 @@
 #include "homg_visit3.cuh"
 #include "homg_moves.cuh"
 #include "homg_literal.cuh"
+#include "homg_pow2.cuh"
 
 namespace homg {
 
@@ -930,6 +931,40 @@ void rec_literal(Rec& R) {
     const int M = s->levels - 1;
     std::vector<Level>& L = s->L;
     Level& L0 = L[0];
+    if (s->pow2) {
+        // PAPER.md section 3 (homg_pow2.cuh): the residual, then nested full weighting on the four anchored lattices
+        rec_norm<T, ND, VAR>(R, true, true, false);
+        const int N = L0.g.nx;
+        auto srcs = [&](int m) { P2Src<T> q; for (int a = 0; a < 4; ++a) q.p[a] = (const T*)s->p2src[a][m]; return q; };
+        auto dsts = [&](int m) { P2Dst<T> q; for (int a = 0; a < 4; ++a) q.p[a] = (T*)s->p2src[a][m]; return q; };
+        for (int m = 1; m <= M; ++m) {
+            const LevelGeom& gc = L[m].g;
+            const dim3 grid((gc.nx + 31) / 32, (gc.ny + 7) / 8, 4);
+            klaunch(R, k_p2_restrict<T>, grid, blk(), 0, gc, L[m - 1].g, N, m == 1 ? 1 : 0, (const T*)L0.gsrc, srcs(m == 1 ? 1 : m - 1),
+                    dsts(m));
+            R.check(TAG_RESTRICT);
+            R.acct(m - 1, m == 1 ? 4.0 : 4.0, TAG_RESTRICT); R.acct(m, 4.0, TAG_RESTRICT);
+        }
+        int ic = 0, ip = 1, in = 2;
+        R.note(cudaMemsetAsync(L0.rot[ic], 0, L0.n_alloc * sizeof(T), R.st)); R.check(TAG_OTHER);
+        R.note(cudaMemsetAsync(L0.rot[ip], 0, L0.n_alloc * sizeof(T), R.st)); R.check(TAG_OTHER);
+        R.acct(0, 2.0, TAG_OTHER);
+        for (size_t vi = 0; vi < s->sched_lv.size(); ++vi) {
+            const int m = s->sched_lv[vi];
+            for (int it = 0; it < s->sched_it[vi]; ++it) {
+                klaunch(R, k_iter_p2<T>, grd(L0.g), blk(), 0, L0.g, L[m].g, N, m, make_coef<T>(s, m), (const T*)L0.rot[ic],
+                        (const T*)L0.rot[ip], (T*)L0.rot[in], (const T*)L0.gsrc, srcs(m == 0 ? 1 : m));
+                R.check(m == 0 ? TAG_RELAX0 : TAG_RELAX);
+                R.acct(0, 3.0, m == 0 ? TAG_RELAX0 : TAG_RELAX);
+                const int t = ip; ip = ic; ic = in; in = t;
+            }
+        }
+        const long long n16 = (long long)(L0.n_alloc * sizeof(T) / 16);
+        klaunch(R, k_add_v<T>, dim3((unsigned)((n16 + 255) / 256)), dim3(256), 0, (T*)s->u, (const T*)L0.rot[ic], n16);
+        R.check(TAG_OTHER);
+        R.acct(0, 3.0, TAG_OTHER);
+        return;
+    }
     const bool have_g1 = rec_norm<T, ND, VAR>(R, true, true, true);           // r -> g_0, norm, g_1
     for (int m = have_g1 ? 2 : 1; m <= M; ++m) {
         klaunch(R, k_restrict<T, ND>, grd(L[m].g), blk(), 0, L[m].g, L[m - 1].g, (const T*)L[m - 1].gsrc, (T*)L[m].gsrc);

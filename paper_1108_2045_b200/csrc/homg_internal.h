@@ -42,6 +42,7 @@ struct Level {
 struct Plan {                  // result of plan_layout: sizes only, no pointers
     int ndim = 0, levels = 0, esize = 0;
     bool var = false;
+    bool pow2 = false;         // HOMG_POISSON5_POW2: level m >= 1 holds the four anchored source arrays only
     std::vector<LevelGeom> g;
     std::vector<size_t> n_alloc;
     size_t staging_bytes = 0;  // dense level-0 array for pack/unpack
@@ -80,6 +81,8 @@ struct homg_solver {
     homg_solver* inner = nullptr;    // mixed precision: this is the fp64 outer problem (1 level), inner the
                                      // fp32 hierarchy that runs the correction cycle; owned by this object
     bool literal = false;            // paper-literal whole-grid iteration, Algorithm L
+    bool pow2 = false;               // PAPER.md section 3: power-of-two grid (whole-grid iteration, homg_pow2.cuh)
+    void* p2src[4][homg::kMaxLevels] = {};   // restricted sources on the four anchored lattices, levels >= 1
     bool vcycle = false;             // classic V(v_eta1, v_eta2) instead of the MFMG cycle
     int v_eta1 = 2, v_eta2 = 1;
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)

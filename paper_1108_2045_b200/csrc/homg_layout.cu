@@ -19,14 +19,22 @@ bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, hom
     if (dt != HOMG_F32 && dt != HOMG_F64) return fail("dtype must be HOMG_F32 or HOMG_F64");
     if (st == HOMG_POISSON5 && ndim != 2) return fail("HOMG_POISSON5 needs ndim = 2");
     if ((st == HOMG_POISSON7 || st == HOMG_DIFFUSION7) && ndim != 3) return fail("7-point stencils need ndim = 3");
-    if (st != HOMG_POISSON5 && st != HOMG_POISSON7 && st != HOMG_DIFFUSION7) return fail("unknown stencil");
+    if (st == HOMG_POISSON5_POW2 && ndim != 2) return fail("HOMG_POISSON5_POW2 needs ndim = 2");
+    if (st != HOMG_POISSON5 && st != HOMG_POISSON7 && st != HOMG_DIFFUSION7 && st != HOMG_POISSON5_POW2) return fail("unknown stencil");
     int64_t q = int64_t(1) << (levels - 1);
-    for (int a = 0; a < ndim; ++a) {
+    const bool pow2 = st == HOMG_POISSON5_POW2;
+    if (pow2) {
+        // PAPER.md section 3: N = 2^k nodes per side; the coarsest lattice of a half is {anchor, central point}: l <= N/2
+        const int64_t N = dims[0];
+        if (dims[1] != N || N < 8 || N > (int64_t(1) << 15) || (N & (N - 1)) != 0) return fail("HOMG_POISSON5_POW2: dims = (N, N), N = 2^k, 8 <= N <= 32768");
+        if (q > N / 2) return fail("HOMG_POISSON5_POW2: 2^(levels-1) must not exceed N/2");
+    }
+    for (int a = 0; a < ndim && !pow2; ++a) {
         if (dims[a] < 3 || dims[a] > (int64_t(1) << 30)) return fail("dims out of range");
         if ((dims[a] - 1) % q != 0 || (dims[a] - 1) / q < 2)
             return fail("every dims[a] must equal c*2^(levels-1)+1 with c >= 2");
     }
-    P.ndim = ndim; P.levels = levels; P.esize = int(dt); P.var = (st == HOMG_DIFFUSION7);
+    P.ndim = ndim; P.levels = levels; P.esize = int(dt); P.var = (st == HOMG_DIFFUSION7); P.pow2 = pow2;
     P.g.clear(); P.n_alloc.clear();
     size_t es = size_t(dt);
     size_t row_align = 128 / es;           // elements per 128 B
@@ -35,6 +43,7 @@ bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, hom
         LevelGeom g;
         int64_t n[3] = {1, 1, 1};
         for (int a = 0; a < ndim; ++a) n[3 - ndim + a] = ((dims[a] - 1) >> m) + 1;
+        if (pow2 && m >= 1) n[1] = n[2] = (dims[0] >> m) + 1;            // an anchored lattice of the (N+1)-node grid
         g.nz = int(n[0]); g.ny = int(n[1]); g.nx = int(n[2]);
         g.px = int(round_up(size_t(g.nx), row_align));
         g.pp = (long long)g.px * g.ny;
@@ -43,7 +52,8 @@ bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, hom
         P.g.push_back(g);
         P.n_alloc.push_back(na);
         size_t arrays;
-        if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 4 : 0) /*k fz fy fx*/;
+        if (pow2 && m >= 1) arrays = 4;                                   // the four anchored source arrays
+        else if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 4 : 0) /*k fz fy fx*/;
         else arrays = kNumRot + 4 /*a g d0 tmp*/ + (P.var ? 4 : 0);
         total += arrays * na * es;
     }

@@ -11,9 +11,10 @@ LIB_PATH = os.path.join(HERE, "libhomg.so")
 
 HOMG_OK, HOMG_EINVAL, HOMG_ENOMEM, HOMG_ECUDA, HOMG_ESTATE = range(5)
 HOMG_F32, HOMG_F64 = 4, 8
-HOMG_POISSON5, HOMG_POISSON7, HOMG_DIFFUSION7 = 0, 1, 2
+HOMG_POISSON5, HOMG_POISSON7, HOMG_DIFFUSION7, HOMG_POISSON5_POW2 = 0, 1, 2, 3
 HOMG_SCHED_C, HOMG_SCHED_A, HOMG_SCHED_SAWTOOTH, HOMG_SCHED_EXPLICIT = 0, 1, 2, 3
-STENCILS = {"poisson5": HOMG_POISSON5, "poisson7": HOMG_POISSON7, "diffusion7": HOMG_DIFFUSION7}
+STENCILS = {"poisson5": HOMG_POISSON5, "poisson7": HOMG_POISSON7, "diffusion7": HOMG_DIFFUSION7,
+            "poisson5_pow2": HOMG_POISSON5_POW2}
 DTYPES = {"f32": HOMG_F32, "f64": HOMG_F64}
 
 # every symbol include/homg.h declares (tests check that the library exports each one)

@@ -573,3 +573,64 @@ def test_a_cycle_is_one_graph_of_kernels_and_memsets_only():
             assert c["memcpy"] == 0 and c["other"] == 0, (name, which, c)
             assert c["conditional"] == which
         s.destroy()
+
+
+# ---- PAPER.md section 3: power-of-two grids (HOMG_POISSON5_POW2, homg_pow2.cuh) vs the oracle's Algorithm P ----
+@pytest.mark.parametrize("N,dtype,levels,kind,maxi,fkind", [(16, "f64", 4, 0, 4, "sine"), (32, "f64", 5, 0, 2, "noise"),
+                                                           (64, "f64", 6, 1, 4, "noise"), (64, "f64", 4, 2, 8, "sine"),
+                                                           (128, "f32", 7, 0, 4, "noise"), (256, "f64", 8, 0, 4, "noise"),
+                                                           (1024, "f64", 10, 0, 4, "noise"), (512, "f32", 9, 0, 32, "sine")])
+def test_pow2_grids(orc, N, dtype, levels, kind, maxi, fkind):
+    _torch()
+    from paper_1108_2045_b200 import homg
+    npdt = np.float64 if dtype == "f64" else np.float32
+    f = I.sine_rhs((N, N)) + I.uniform_field((N, N), 11, -1e-3, 1e-3) if fkind == "sine" else I.normal_field((N, N), 12)
+    f = np.ascontiguousarray(f, dtype=npdt)
+    u0 = np.ascontiguousarray(I.uniform_field((N, N), 13, -1.0, 1.0) if fkind == "noise" else np.zeros((N, N)), dtype=npdt)
+    ncyc = 3
+    s = homg.Solver((N, N), levels, "poisson5_pow2", dtype, omega=0.8, max_iters=maxi, schedule=kind)
+    s.set_rhs(f)
+    s.set_initial_guess(u0)
+    us = []
+    for _ in range(ncyc):
+        s.cycle(1)
+        us.append(s.get_solution().copy())
+    norms = np.array(s.residual_history() + [s.residual_norm()[0]])
+    sched = s.schedule()
+    osched = orc.schedule(kind, levels, maxi)
+    assert (list(sched[0]), list(sched[1])) == (list(osched[0]), list(osched[1]))
+    s.destroy()
+    _, hist, onorms = orc.homg_p2(f, u0, levels, 0.8, osched, ncyc)
+    for c in range(ncyc):
+        ref = hist[c].astype(np.float64)
+        err = np.max(np.abs(us[c].astype(np.float64) - ref)) / np.max(np.abs(ref))
+        assert err <= TOL[dtype], f"pow2 N={N}: cycle {c}: {err:.3e}"
+    assert np.allclose(norms, onorms, rtol=1e-5 if dtype == "f32" else 1e-10)
+    for ax in range(2):
+        assert not np.any(np.take(us[-1], [0, -1], axis=ax))
+
+
+def test_pow2_converges_at_a_grid_independent_rate_and_argument_checks():
+    """PAPER.md L85 on the GPU: with the central points the residual contracts by the same factor per cycle on every
+    power-of-two grid (the oracle pin P12f: < 0.30)."""
+    _torch()
+    from paper_1108_2045_b200 import homg
+    facs = []
+    for N in (64, 256, 1024):
+        k = int(np.log2(N))
+        f = np.ascontiguousarray(I.sine_rhs((N, N)))
+        s = homg.Solver((N, N), k, "poisson5_pow2", "f64", omega=0.8)
+        s.set_rhs(f)
+        s.cycle(8)
+        h = s.residual_history()
+        facs.append(h[7] / h[6])
+        s.destroy()
+    assert max(facs) < 0.30 and max(facs) - min(facs) < 0.05, facs
+    with pytest.raises(homg.HomgError):
+        homg.Solver((64, 64), 7, "poisson5_pow2", "f64")            # l = 64 > N/2
+    with pytest.raises(homg.HomgError):
+        homg.Solver((65, 65), 5, "poisson5_pow2", "f64")
+    with pytest.raises(homg.HomgError):
+        homg.Solver((64, 32), 4, "poisson5_pow2", "f64")
+    with pytest.raises(homg.HomgError):
+        homg.Solver((64, 64), 5, "poisson5_pow2", "f64", vcycle=(2, 1))
