@@ -220,6 +220,25 @@ HOMG_API const char* homg_tag_name(int tag);
  * in the per-sweep count of SURVEY.md 8(d)) in one pass.  Valid after the first homg_cycle. */
 HOMG_API double homg_compulsory_bytes_per_cycle(const homg_solver* s, double* bytes_by_tag, int cap);
 
+/* The ONE entry point that allocates nothing (csrc/homg_noalloc.cu) — for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it) and hence cannot give a
+ * homg_solver its workspace.  The residual-norm step (r = f - A u, ||r||_2 over the interior nodes,
+ * accumulated in fp64; A = -lap, 5-point for ndim = 2, 7-point for ndim = 3, mesh width h, h <= 0: 1/(dims[0]-1))
+ * of DENSE C-order DEVICE arrays u_dev, f_dev of prod(dims) scalars of `dtype` (dims as everywhere: nodes incl. the
+ * boundary, dims[0] slowest).  Boundary entries of u must hold the Dirichlet value 0 (as homg_get_solution returns
+ * them); those of f are ignored.  *norm_out_dev (a DEVICE double, caller-owned) receives ||r||_2, asynchronously on
+ * cuda_stream (NULL = the legacy default stream); nothing is copied to the host and nothing is synchronised.
+ * The per-block partial sums live in a static __device__ array of 131072 doubles (1 MiB, held by every GPU that
+ * loads the library until the process exits): a grid with ceil(nx/32) * ceil(ny/8) * nz > 131072 (above 257^3 or
+ * 4097^2) is rejected with HOMG_EINVAL.  No cudaMalloc, cudaFree or allocating library routine is called.
+ * Every call shares that array: CALLS THAT OVERLAP ON THE GPU (different streams or threads) RACE — serialise
+ * them.  Nothing in it needs to start at zero (every block writes its entry; the array keeps the last call's
+ * contents).  err (nullable, err_cap bytes) receives the text of an error.  The same value as homg_residual_norm of
+ * a solver holding the same u and f, up to the order of the fp64 summation. */
+HOMG_API homg_status homg_residual_norm_noalloc(int ndim, const int64_t* dims, homg_dtype dtype, double h,
+                                                const void* u_dev, const void* f_dev, double* norm_out_dev,
+                                                void* cuda_stream, char* err, size_t err_cap);
+
 HOMG_API void homg_destroy(homg_solver* s);
 
 /* Text of the last error on this solver ("" if none).  s may be NULL: returns the text

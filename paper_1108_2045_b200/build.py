@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhomg.so")
-SOURCES = ["homg_layout.cu", "homg_exec.cu", "homg_api.cu"]
+SOURCES = ["homg_layout.cu", "homg_exec.cu", "homg_api.cu", "homg_noalloc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 # -fmad=false: the kernels evaluate exactly the expression trees DESIGN.md states (the same ones the
 # oracle is compiled to with -ffp-contract=off), so fp64 AND fp32 results agree with it bit for bit;

@@ -22,6 +22,7 @@ SYMBOLS = [
     "homg_default_options", "homg_workspace_bytes", "homg_create", "homg_set_rhs", "homg_set_initial_guess",
     "homg_set_coefficient", "homg_cycle", "homg_solve", "homg_residual_norm", "homg_residual_history", "homg_get_solution",
     "homg_profile_cycles", "homg_tag_name", "homg_compulsory_bytes_per_cycle", "homg_workspace_bytes_mixed", "homg_get_schedule", "homg_launches_per_cycle", "homg_graph_nodes", "homg_bytes_per_cycle", "homg_destroy", "homg_last_error",
+    "homg_residual_norm_noalloc",
 ]
 
 
@@ -73,6 +74,8 @@ def lib():
         L.homg_tag_name.argtypes = [i]; L.homg_tag_name.restype = C.c_char_p
         L.homg_compulsory_bytes_per_cycle.argtypes = [vp, C.POINTER(d), i]; L.homg_compulsory_bytes_per_cycle.restype = d
         L.homg_destroy.argtypes = [vp]; L.homg_destroy.restype = None
+        L.homg_residual_norm_noalloc.argtypes = [i, i64p, i, d, vp, vp, vp, vp, C.c_char_p, C.c_size_t]
+        L.homg_residual_norm_noalloc.restype = i
         L.homg_last_error.argtypes = [vp]; L.homg_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -95,6 +98,26 @@ def _ptr_and_flag(x):
     if not x.flags["C_CONTIGUOUS"]:
         raise ValueError("array must be C-contiguous")
     return x.ctypes.data, 0
+
+
+def residual_norm_noalloc(u, f, out, h=0.0, stream=None):
+    """homg_residual_norm_noalloc: ||f - A u||_2 of dense CUDA tensors u, f (same shape and dtype, boundary of u = 0)
+    into the caller's CUDA float64 tensor `out` (>= 1 element), asynchronously; no allocation by the library (its
+    scratch is a static device array: calls that overlap on the GPU race).  Marshalling only."""
+    import torch
+    if not (u.is_cuda and f.is_cuda and out.is_cuda) or out.dtype != torch.float64 or out.numel() < 1:
+        raise ValueError("u, f: CUDA tensors; out: a CUDA float64 tensor")
+    if u.shape != f.shape or u.dtype != f.dtype or not (u.is_contiguous() and f.is_contiguous()):
+        raise ValueError("u and f must be contiguous tensors of the same shape and dtype")
+    dt = {torch.float32: HOMG_F32, torch.float64: HOMG_F64}[u.dtype]
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(u.device):
+        st = stream if stream is not None else torch.cuda.current_stream(u.device)
+        rc = lib().homg_residual_norm_noalloc(u.dim(), _dims(tuple(u.shape)), dt, float(h), C.c_void_p(u.data_ptr()),
+                                              C.c_void_p(f.data_ptr()), C.c_void_p(out.data_ptr()),
+                                              C.c_void_p(st.cuda_stream), err, len(err))
+    if rc != HOMG_OK:
+        raise HomgError(rc, err.value.decode())
 
 
 class Solver:
