@@ -221,6 +221,7 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     if (const char* ev = std::getenv("HOMG_FUSE_FIRST_VAR")) s->fuse_first_var = std::atoi(ev) != 0;
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_VISIT3")) s->visit3 = std::atoi(ev);
+    if (const char* ev = std::getenv("HOMG_BRICKS")) s->bricks = std::atoi(ev) != 0;
     s->vcycle = o.cycle == HOMG_CYCLE_V;
     s->pow2 = P.pow2;
     s->literal = o.cycle == HOMG_CYCLE_LITERAL || P.pow2;

@@ -15,6 +15,7 @@
 #include "homg_visit.cuh"
 #include "homg_visit3.cuh"
 #include "homg_moves.cuh"
+#include "homg_bricks.cuh"
 #include "homg_literal.cuh"
 #include "homg_pow2.cuh"
 
@@ -131,6 +132,12 @@ int resident_ctas(K kern, int threads, size_t smem) {
     return n;
 }
 
+// level-change kernels: the brick form (homg_bricks.cuh: 2 x 2 fine rows per thread) pays on large fine levels
+// (measured: cfg4 1.379 -> 1.366 ms per cycle, cfg5 deliver onto level 0 63 -> 43 us); on small ones its 4 x fewer
+// threads cost more latency than the saved loads (cfg2 0.165 -> 0.1725): one pack per thread below 10^6 nodes
+inline bool use_bricks(const homg_solver* s, const LevelGeom& gf) {
+    return s->bricks && (long long)gf.nx * gf.ny * gf.nz >= 1000000LL;
+}
 inline dim3 blk() { return dim3(32, 8, 1); }
 inline dim3 grd(const LevelGeom& g) { return dim3((g.nx + 31) / 32, (g.ny + 7) / 8, g.nz); }
 template <class T>
@@ -578,7 +585,7 @@ void rec_cycle(Rec& R) {
                         pend[m] = PendingDeliver{true, rotp<T>(Lc, Lc.e), ac, rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode};
                     } else {
                         flush();
-                        if (!R.plan) klaunch(R, k_deliver_v<T, ND>, grdv<T>(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
+                        if (!R.plan) klaunch(R, use_bricks(R.s, Lf.g) ? k_deliver_b<T, ND> : k_deliver_v<T, ND>, use_bricks(R.s, Lf.g) ? grdb<T, ND>(Lf.g) : grdv<T>(Lf.g), blk(), 0, Lf.g, Lc.g, rotp<T>(Lc, Lc.e), ac,
                                                                                     rotp<T>(Lf, Lf.e), (T*)Lf.a, ef_assign, af_mode);
                         R.check(tag);
                     }
@@ -647,13 +654,13 @@ void rec_cycle(Rec& R) {
                         } else if (pend[m].on) {
                             flush();
                             const PendingDeliver& pd = pend[m];
-                            if (!R.plan) klaunch(R, k_arrive_v<T, ND>, grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, pd.ec, pd.ac, pd.ef,
+                            if (!R.plan) klaunch(R, use_bricks(R.s, L[m - 1].g) ? k_arrive_b<T, ND> : k_arrive_v<T, ND>, use_bricks(R.s, L[m - 1].g) ? grdb<T, ND>(L[m - 1].g) : grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, pd.ec, pd.ac, pd.ef,
                                                  pd.af, pd.ef_assign, pd.af_mode, A, B, out, last ? (1 << (cur - t)) : 0,
                                                  last ? cur - t : 0, Lv.g, X, Y);
                             R.check(TAG_DELIVER);
                         } else {
                             flush();
-                            if (!R.plan) klaunch(R, k_d0_down_v<T, ND>, grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,
+                            if (!R.plan) klaunch(R, use_bricks(R.s, L[m - 1].g) ? k_d0_down_b<T, ND> : k_d0_down_v<T, ND>, use_bricks(R.s, L[m - 1].g) ? grdb<T, ND>(L[m - 1].g) : grdv<T>(L[m - 1].g), blk(), 0, L[m - 1].g, L[m].g, A, B, out,
                                                                                                 last ? (1 << (cur - t)) : 0, last ? cur - t : 0, Lv.g, X, Y);
                             R.check(tag);
                         }
@@ -907,7 +914,7 @@ void rec_vcycle(Rec& R) {
     }
     for (int m = M - 1; m >= 0; --m) {
         Level& Lm = L[m];
-        klaunch(R, k_prolong_add_v<T, ND>, grdv<T>(Lm.g), blk(), 0, Lm.g, L[m + 1].g, (const T*)cur[m + 1], cur[m]);   // (d)
+        klaunch(R, use_bricks(R.s, Lm.g) ? k_prolong_add_b<T, ND> : k_prolong_add_v<T, ND>, use_bricks(R.s, Lm.g) ? grdb<T, ND>(Lm.g) : grdv<T>(Lm.g), blk(), 0, Lm.g, L[m + 1].g, (const T*)cur[m + 1], cur[m]);   // (d)
         R.check(m == 0 ? TAG_DELIVER0 : TAG_DELIVER);
         R.acct(m, 2.0, m == 0 ? TAG_DELIVER0 : TAG_DELIVER); R.acct(m + 1, 1.0, m == 0 ? TAG_DELIVER0 : TAG_DELIVER);
         R.g_override = m == 0 ? s->f : nullptr;

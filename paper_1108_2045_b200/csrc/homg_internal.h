@@ -88,6 +88,7 @@ struct homg_solver {
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
     int visit3 = 2;                  // 3-D K_visit: 2 = homg_visit3.cuh for every form (default); 1 = only the level-0 / plain
                                      // forms, bookkeeping visits on homg_visit.cuh; 0 = homg_visit.cuh (the r01 kernel) throughout
+    bool bricks = true;              // level-change kernels in brick form (homg_bricks.cuh); HOMG_BRICKS=0: one pack per thread
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create
     std::vector<int> sched_lv, sched_it;

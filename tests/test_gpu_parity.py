@@ -634,3 +634,19 @@ def test_pow2_converges_at_a_grid_independent_rate_and_argument_checks():
         homg.Solver((64, 32), 4, "poisson5_pow2", "f64")
     with pytest.raises(homg.HomgError):
         homg.Solver((64, 64), 5, "poisson5_pow2", "f64", vcycle=(2, 1))
+
+
+def test_brick_and_pack_level_change_kernels_agree_bitwise(orc, monkeypatch):
+    """homg_bricks.cuh (2 x 2 fine rows per thread, used on fine levels of >= 10^6 nodes) against homg_moves.cuh (one
+    pack per thread): same arithmetic term by term, hence the same bits — 3-D fp32 / fp64, 2-D, and the V cycle."""
+    import dataclasses
+    for name, n, kw in (("cfg4", 129, {}), ("cfg5", 129, {}), ("cfg3", 2049, {}), ("cfg4", 129, {"vcycle": (2, 1)})):
+        cfg = dataclasses.replace(I.scaled(I.CONFIGS[name], n))
+        inp = I.make_inputs(cfg)
+        monkeypatch.setenv("HOMG_BRICKS", "1")
+        a, na, _ = run_gpu(cfg, inp, 2, **kw)
+        monkeypatch.setenv("HOMG_BRICKS", "0")
+        b, nb, _ = run_gpu(cfg, inp, 2, **kw)
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y), (name, n, kw)
+        assert np.array_equal(na, nb)
