@@ -222,6 +222,7 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
     if (const char* ev = std::getenv("HOMG_FUSE_VISIT")) s->fuse_visit = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_VISIT3")) s->visit3 = std::atoi(ev);
     if (const char* ev = std::getenv("HOMG_BRICKS")) s->bricks = std::atoi(ev) != 0;
+    if (const char* ev = std::getenv("HOMG_VISIT_VAR")) s->visit_var = std::atoi(ev) != 0;
     s->vcycle = o.cycle == HOMG_CYCLE_V;
     s->pow2 = P.pow2;
     s->literal = o.cycle == HOMG_CYCLE_LITERAL || P.pow2;
@@ -267,7 +268,7 @@ static homg_status create_one(homg_solver** out, int ndim, const int64_t* dims, 
         L.gsrc = take(ab);
         for (int b = 0; b < L.nrot; ++b) L.rot[b] = take(ab);
         if (m >= 1) { L.a = take(ab); L.d0 = take(ab); L.tmp = take(ab); }
-        if (P.var) { L.k = take(ab); L.fz = take(ab); L.fy = take(ab); L.fx = take(ab); }
+        if (P.var) { L.k = take(ab); L.fz = take(ab); L.fy = take(ab); L.fx = take(ab); L.wd = take(ab); }
     }
     s->staging = take(P.staging_bytes);
     s->partial = static_cast<double*>(take(P.partial_count * sizeof(double)));

@@ -318,13 +318,13 @@ void launch_visit(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T
 }
 
 // K_visit, 3-D form (homg_visit3.cuh): two rows per thread, g carried in registers
-template <class T, int NS, bool INTERP, bool BOOK>
+template <class T, int NS, bool INTERP, bool BOOK, bool VAR = false>
 void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
                     const T* d0, const T* v0, T* u) {
     homg_solver* s = R.s;
     Level& Lt = s->L[t];
-    using TL = Visit3Tile<T, NS, BOOK>;
-    CUtensorMap tm_in, tm_ac, tm_g, tm_u;
+    using TL = Visit3Tile<T, NS, BOOK, VAR>;
+    CUtensorMap tm_in, tm_ac, tm_g, tm_u, tm_fz, tm_fy, tm_fx, tm_wd;
     bool ok = make_tmap<T, 3>(s, &tm_g, R.g_override ? R.g_override : Lt.gsrc, Lt.g, TL::TXN, TL::PY);
     if (INTERP) {
         Level& Lc = s->L[t + 1];
@@ -335,6 +335,12 @@ void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0,
     }
     if (u && !BOOK) ok = ok && make_tmap<T, 3>(s, &tm_u, u, Lt.g, TL::OX, TL::OY);
     else tm_u = tm_g;
+    if (VAR) {
+        ok = ok && make_tmap<T, 3>(s, &tm_fz, Lt.fz, Lt.g, TL::TXN, TL::PY) && make_tmap<T, 3>(s, &tm_fy, Lt.fy, Lt.g, TL::TXN, TL::PY) &&
+             make_tmap<T, 3>(s, &tm_fx, Lt.fx, Lt.g, TL::TXN, TL::PY) && make_tmap<T, 3>(s, &tm_wd, Lt.wd, Lt.g, TL::TXN, TL::PY);
+    } else {
+        tm_fz = tm_fy = tm_fx = tm_wd = tm_g;
+    }
     if (!ok) { if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue; return; }
     const LevelGeom& g = Lt.g;
     const int interior = std::max(g.nz - 2, 1);
@@ -355,8 +361,8 @@ void launch_visit3b(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0,
     mc = (mc + 1) & ~1;
     const int nch = (interior + mc - 1) / mc;
     dim3 grid(tx, ty, nch);
-    klaunch(R, k_visit3<T, NS, INTERP, BOOK>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP, BOOK>(), tm_in, tm_ac, tm_g, tm_u, g,
-            make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
+    klaunch(R, k_visit3<T, NS, INTERP, BOOK, VAR>, grid, TL::NT, visit3_smem_bytes<T, NS, INTERP, BOOK, VAR>(), tm_in, tm_ac, tm_g, tm_u,
+            tm_fz, tm_fy, tm_fx, tm_wd, g, make_coef<T>(s, t), o0, o1, o2, a, a_assign, d0, v0, u, mc);
 }
 template <class T, int NS, bool INTERP>
 void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a, int a_assign,
@@ -365,9 +371,14 @@ void launch_visit3(Rec& R, int t, const T* in, const T* ec, const T* ac, T* o0, 
     else launch_visit3b<T, NS, INTERP, false>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
 }
 
-template <class T, int ND, bool INTERP>
+template <class T, int ND, bool INTERP, bool VAR = false>
 void launch_visit_ns(Rec& R, int ns, int t, const T* in, const T* ec, const T* ac, T* o0, T* o1, T* o2, T* a,
                      int a_assign, const T* d0, const T* v0, T* u) {
+    if (VAR) {                                    // variable coefficient: 3-D, level-0 form, two sweeps per pass
+        if (ND == 3 && ns == 2 && !(a || o1 || o2)) launch_visit3b<T, 2, INTERP, false, ND == 3 && VAR>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
+        else if (R.err == cudaSuccess) R.err = cudaErrorInvalidValue;
+        return;
+    }
     // (visit3 == 1 keeps the S3e-bookkeeping form of levels >= 1 on homg_visit.cuh)
     if (ND == 3 && R.s->visit3 && (R.s->visit3 >= 2 || INTERP || !(a || o1 || o2))) {
         if (ns == 2) launch_visit3<T, 2, INTERP>(R, t, in, ec, ac, o0, o1, o2, a, a_assign, d0, v0, u);
@@ -535,10 +546,13 @@ void rec_cycle(Rec& R) {
         // K_visit runs this visit (decided here because a level-0 visit in MID-cycle must leave v^{eta-1} behind for
         // the carried variation of the next visit: K_visit stores it only in its bookkeeping form, which takes its
         // v^0 from memory — such a visit is not fused with its arrival)
-        const int kv_maxns = std::min(s->fuse_visit, 4);
-        const bool use_kvisit = !VAR && kv_maxns >= 2 && tiled(s, t) && !(s->coarse_threshold > 0 && Lt.n_nodes <= s->coarse_threshold) &&
-                                eta >= 2 && (t == 0 || eta <= kv_maxns);
+        // (variable coefficient, 8(f)4b: K_visit's level-0 form only, two sweeps per pass, when visit_var is on; not in the
+        // fp32 inner cycle of the mixed-precision loop, whose parity with the mixed oracle rests on bit-exact sweeps)
+        const int kv_maxns = VAR ? 2 : std::min(s->fuse_visit, 4);
         const bool mid_l0 = t == 0 && vi != nv - 1;
+        const bool use_kvisit = (VAR ? (ND == 3 && s->visit_var && !s->given_g0 && s->visit3 && t == 0 && !mid_l0) : true) && std::min(s->fuse_visit, 4) >= 2 &&
+                                tiled(s, t) && !(s->coarse_threshold > 0 && Lt.n_nodes <= s->coarse_threshold) &&
+                                eta >= 2 && (t == 0 || eta <= kv_maxns);
         if (cur < 0) {
             if (small(t)) {
                 CoarseOp<T> o = newop(OP_ZERO, t);
@@ -564,7 +578,7 @@ void rec_cycle(Rec& R) {
                     Level& Lc = L[m];
                     Level& Lf = L[m - 1];
                     int ef_assign = Lf.touched ? 0 : 1;
-                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && (VAR ? s->fuse_first_var : s->fuse_first) &&
+                    if (m - 1 == t && t == 0 && ef_assign && !a_zero[m] && tiled(s, t) && (VAR ? (s->fuse_first_var || use_kvisit) : s->fuse_first) &&
                         !(use_kvisit && mid_l0)) {
                         fuse_first = true;                   // S3a of this hop happens inside the first sweep
                         fuse_ec = rotp<T>(Lc, Lc.e);
@@ -713,10 +727,10 @@ void rec_cycle(Rec& R) {
                 const int tag = t == 0 ? TAG_VISIT0 : TAG_VISIT;
                 if (!R.plan) {
                     if (interp)
-                        launch_visit_ns<T, ND, true>(R, ns, t, nullptr, fuse_ec, (const T*)L[t + 1].a, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                        launch_visit_ns<T, ND, true, VAR>(R, ns, t, nullptr, fuse_ec, (const T*)L[t + 1].a, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
                                                   nullptr, 0, nullptr, nullptr, addu ? (T*)s->u : nullptr);
                     else
-                        launch_visit_ns<T, ND, false>(R, ns, t, rotp<T>(Lt, in), nullptr, nullptr, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
+                        launch_visit_ns<T, ND, false, VAR>(R, ns, t, rotp<T>(Lt, in), nullptr, nullptr, o0, rotp<T>(Lt, b1), rotp<T>(Lt, b2),
                                                    book ? (T*)Lt.a : nullptr, a_zero[t] ? 1 : 0, (book && have_d0) ? (const T*)Lt.d0 : nullptr,
                                                    rotp<T>(Lt, v0i), addu ? (T*)s->u : nullptr);
                 }
@@ -728,7 +742,7 @@ void rec_cycle(Rec& R) {
                     const double comp = (interp ? 0.0 : 1.0) + 1.0 + (o0 ? 1.0 : 0.0) + (b1 >= 0 ? 1.0 : 0.0) +
                                         (b2 >= 0 ? 1.0 : 0.0) + bk + (addu ? 2.0 : 0.0);
                     const double alg = (interp ? 2.0 : 3.0) + 3.0 * (ns - 1) + (addu ? 1.0 : 0.0) + bk + (book ? 1.0 : 0.0);
-                    R.acct2(t, alg, comp, tag);
+                    R.acct2(t, alg + (VAR ? 3.0 * ns : 0.0), comp + (VAR ? 4.0 : 0.0), tag);   // + the three face arrays (+ omega/D in the fused form)
                 }
                 // rot indices of the last three iterates
                 if (ns >= 3) { i2 = b2; i1 = b1; }
@@ -1010,6 +1024,10 @@ void rec_sample(Rec& R) {
         Level& Lm = s->L[m];
         klaunch(R, k_faces<T, ND>, grd(Lm.g), blk(), 0, Lm.g, (const T*)Lm.k, (T*)Lm.fz, (T*)Lm.fy, (T*)Lm.fx);
         R.check(TAG_OTHER);
+        if (Lm.wd) {
+            klaunch(R, k_wdiag<T, ND>, grd(Lm.g), blk(), 0, Lm.g, make_coef<T>(s, m), faces<T>(Lm), (T*)Lm.wd);
+            R.check(TAG_OTHER);
+        }
     }
 }
 
@@ -1090,7 +1108,11 @@ cudaError_t set_attr_visit() {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k_visit3<T, NS, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, false, true>());
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_visit3<T, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, true, false>());
+    e = cudaFuncSetAttribute(k_visit3<T, NS, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, NS, true, false>());
+    if (e != cudaSuccess || NS != 2) return e;
+    e = cudaFuncSetAttribute(k_visit3<T, 2, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, 2, false, false, true>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_visit3<T, 2, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, visit3_smem_bytes<T, 2, true, false, true>());
 }
 
 }  // namespace

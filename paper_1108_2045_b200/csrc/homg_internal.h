@@ -32,6 +32,7 @@ struct Level {
     void* fz = nullptr;        // face coefficients towards +z / +y / +x (HOMG_DIFFUSION7; homg_geom.h Faces)
     void* fy = nullptr;
     void* fx = nullptr;
+    void* wd = nullptr;        // omega / D per node, D = the operator's diagonal (HOMG_DIFFUSION7; S0; read by K_visit's variable-coefficient form)
     // --- executor state while one cycle is being recorded ---
     int e = 0;                 // rot index holding the materialised correction e_m
     bool touched = false;      // e_m / a_m already defined in this cycle
@@ -88,6 +89,8 @@ struct homg_solver {
     int fuse_visit = 4;              // K_visit: up to this many sweeps of a visit in one pass (0/1: off; HOMG_FUSE_VISIT)
     int visit3 = 2;                  // 3-D K_visit: 2 = homg_visit3.cuh for every form (default); 1 = only the level-0 / plain
                                      // forms, bookkeeping visits on homg_visit.cuh; 0 = homg_visit.cuh (the r01 kernel) throughout
+    bool visit_var = true;           // K_visit for the variable-coefficient stencil: level 0, two sweeps per pass, multiplies by the
+                                     // precomputed RN(omega/D) (rounding-level difference to the per-sweep kernels); HOMG_VISIT_VAR=0: per sweep
     bool bricks = true;              // level-change kernels in brick form (homg_bricks.cuh); HOMG_BRICKS=0: one pack per thread
     int sm_count = 148;
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, fetched from the driver at create

@@ -409,6 +409,22 @@ __global__ void k_faces(LevelGeom g, const T* __restrict__ k, T* __restrict__ fz
     if (ND == 3) fz[c] = z + 1 < g.nz ? kface(kc, k[c + g.pp]) : T(0);
 }
 
+// S0: wd = omega / D at every interior node, D = (sum of the 2d face coefficients) / h^2 summed in the sweep's own order
+// (z-, z+, y-, y+, x-, x+), so that D is the very number the sweeps compute; 0 on the boundary.  Read by the
+// variable-coefficient form of K_visit, which then needs neither the sum nor the division per sweep (R14).
+template <class T, int ND>
+__global__ void k_wdiag(LevelGeom g, Coef<T> cf, Faces<T> kf, T* __restrict__ wd) {
+    pdl_start();
+    HOMG_NODE_XYZ(g);
+    const long long c = lidx(g, x, y, z);
+    if (!is_interior<ND>(g, x, y, z)) { wd[c] = T(0); return; }
+    T ds = T(0);
+    if (ND == 3) { ds += kf.z[c - g.pp]; ds += kf.z[c]; }
+    ds += kf.y[c - g.px]; ds += kf.y[c];
+    ds += kf.x[c - 1]; ds += kf.x[c];
+    wd[c] = cf.w / (ds * cf.ih2);
+}
+
 // coefficient sampling onto the next level: k_c(P) = k_f(2P)     (R11)
 // (same kernel as k_inject; kept under its own name for the profile listing)
 template <class T, int ND>

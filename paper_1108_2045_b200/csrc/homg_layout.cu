@@ -53,8 +53,8 @@ bool plan_layout(int ndim, const int64_t* dims, int levels, homg_stencil st, hom
         P.n_alloc.push_back(na);
         size_t arrays;
         if (pow2 && m >= 1) arrays = 4;                                   // the four anchored source arrays
-        else if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 4 : 0) /*k fz fy fx*/;
-        else arrays = kNumRot + 4 /*a g d0 tmp*/ + (P.var ? 4 : 0);
+        else if (m == 0) arrays = 3 /*rot*/ + 3 /*u f g*/ + (P.var ? 5 : 0) /*k fz fy fx wd*/;
+        else arrays = kNumRot + 4 /*a g d0 tmp*/ + (P.var ? 5 : 0);
         total += arrays * na * es;
     }
     const LevelGeom& g0 = P.g[0];

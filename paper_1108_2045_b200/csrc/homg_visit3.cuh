@@ -26,11 +26,16 @@ namespace homg {
 // BOOK: the visit of a level >= 1 (S3e bookkeeping, three iterates stored) carries more live values per thread
 // (226 registers): 256 threads (16 row pairs, tile 64 x 32) instead of 384 at <= 168.  (320 threads get no more
 // registers than 384: ptxas allots them per group of four warps.)
-template <class T, int NS, bool BOOK>
+// VAR: the variable-coefficient stencil (flux form, R11) keeps three more TMA rings (the face arrays) and
+// more registers per thread: 12 row pairs = 192 threads, tile 16 packs x 24 rows (257^3 fp64: 10 x 13 = 130 tiles)
+#ifndef HOMG_VISIT3_VAR_TR
+#define HOMG_VISIT3_VAR_TR 12
+#endif
+template <class T, int NS, bool BOOK, bool VAR = false>
 struct Visit3Tile {
     static constexpr int ES = int(sizeof(T));
     static constexpr int VEC = 16 / ES;
-    static constexpr int PX = 16, TR = BOOK ? 16 : 24, NT = PX * TR;   // packs per row, row pairs, threads
+    static constexpr int PX = 16, TR = VAR ? HOMG_VISIT3_VAR_TR : (BOOK ? 16 : 24), NT = PX * TR;   // packs per row, row pairs, threads
     static constexpr int HX = (NS + VEC - 1) / VEC * VEC;      // x halo (nodes), pack granular
     static constexpr int HY = (NS + 1) / 2 * 2;                // y halo (rows), row-pair granular
     static constexpr int TXN = PX * VEC, PY = 2 * TR;          // tile in nodes
@@ -60,12 +65,13 @@ struct Visit3Tile {
     static_assert(NIN == UNR && NG == UNR && NC == UNR, "ring slots are compile-time constants of the unrolled loop");
 };
 
-template <class T, int NS, bool INTERP, bool BOOK>
+template <class T, int NS, bool INTERP, bool BOOK, bool VAR = false>
 __host__ __device__ constexpr int visit3_smem_bytes() {
-    using TL = Visit3Tile<T, NS, BOOK>;
+    using TL = Visit3Tile<T, NS, BOOK, VAR>;
     return TL::NG * TL::BOX_BYTES +
            (INTERP ? TL::NC * 2 * TL::CTILE_BYTES + NS * 2 * TL::PLANE_BYTES
-                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + TL::NEP * TL::EP_BYTES + (BOOK ? 0 : TL::NU * TL::UBOX_BYTES) + 128;
+                   : TL::NIN * TL::PLANE_BYTES + (NS - 1) * 2 * TL::PLANE_BYTES) + TL::NEP * TL::EP_BYTES + (BOOK ? 0 : TL::NU * TL::UBOX_BYTES) +
+           (VAR ? 4 * TL::NG * TL::BOX_BYTES : 0) + 128;
 }
 
 // cp.async (LDGSTS): 16 bytes global -> shared without passing through registers; completion per thread
@@ -126,6 +132,38 @@ __device__ __forceinline__ Pack<float> jacobi_pack(const Pack<float>& pv, const 
     return out;
 }
 
+// variable coefficient (flux form, R11/R14): v + (g - A v) wd with A v = sum_faces kf (v - v_nb) / h^2 (faces in the order
+// z-, z+, y-, y+, x-, x+: A v is the very number k_relax_tma<VAR> / the oracle compute) and wd = RN(w / D) precomputed per
+// node in S0 (k_wdiag).  The per-sweep kernels and the oracle evaluate v + w (g - A v) / D: the two differ by rounding only
+// (one multiplication by a rounded quotient instead of a multiplication and a division) — DESIGN.md R14, tolerance 1e-12.
+// Without the sum of the faces and the IEEE division the dependent chain per node is 2.7 x shorter: with 6 warps per SM the
+// kernel is bound by exactly that latency (profiles/r02b).  fxl = the x- face of the pack's first node.
+template <class T>
+__device__ __forceinline__ Pack<T> jacobi_pack_var(const Pack<T>& pv, const Pack<T>& cu, const Pack<T>& nx, const Pack<T>& dn,
+                                                   const Pack<T>& up, const Pack<T>& gv, T vl, T vr, const Pack<T>& wd,
+                                                   const Pack<T>& fzm, const Pack<T>& fzp, const Pack<T>& fym, const Pack<T>& fyp,
+                                                   const Pack<T>& fxp, T fxl, const Coef<T>& cf) {
+    constexpr int VEC = 16 / int(sizeof(T));
+    Pack<T> out;
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+        const T vc = cu.v[j];
+        const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
+        const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+        const T fxm = j == 0 ? fxl : fxp.v[j - 1 < 0 ? 0 : j - 1];
+        T acc = T(0);
+        acc += fzm.v[j] * (vc - pv.v[j]);
+        acc += fzp.v[j] * (vc - nx.v[j]);
+        acc += fym.v[j] * (vc - dn.v[j]);
+        acc += fyp.v[j] * (vc - up.v[j]);
+        acc += fxm * (vc - xm);
+        acc += fxp.v[j] * (vc - xp);
+        const T Av = acc * cf.ih2;
+        out.v[j] = vc + (gv.v[j] - Av) * wd.v[j];                  // wd = 0 on the boundary and outside the grid: v stays 0
+    }
+    return out;
+}
+
 // q mod UNR of a step: a compile-time constant in the steady loop, q itself elsewhere
 template <int N>
 __device__ __forceinline__ constexpr int step_k(std::integral_constant<int, N>) { return N; }
@@ -133,15 +171,20 @@ __device__ __forceinline__ int step_k(int q) { return q; }
 
 // Arguments as k_visit (homg_visit.cuh).  grid = (x tiles of OX, y tiles of OY, z chunks of mchunk interior
 // planes); mchunk must be even when there is more than one chunk (every chunk then starts on an odd plane).
-template <class T, int NS, bool INTERP, bool BOOK>
-__global__ void __launch_bounds__(Visit3Tile<T, NS, BOOK>::NT, 1)
+// VAR: tm_fz / tm_fy / tm_fx = the face arrays of the level (box {TXN, PY, 1} like g); otherwise unused.
+template <class T, int NS, bool INTERP, bool BOOK, bool VAR = false>
+__global__ void __launch_bounds__(Visit3Tile<T, NS, BOOK, VAR>::NT, 1)
 k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_ac,
-         const __grid_constant__ CUtensorMap tm_g, const __grid_constant__ CUtensorMap tm_u, LevelGeom g, Coef<T> cf, T* __restrict__ o0,
+         const __grid_constant__ CUtensorMap tm_g, const __grid_constant__ CUtensorMap tm_u,
+         const __grid_constant__ CUtensorMap tm_fz, const __grid_constant__ CUtensorMap tm_fy,
+         const __grid_constant__ CUtensorMap tm_fx, const __grid_constant__ CUtensorMap tm_wd, LevelGeom g, Coef<T> cf,
+         T* __restrict__ o0,
          T* __restrict__ o1, T* __restrict__ o2, T* __restrict__ a, int a_assign, const T* __restrict__ d0,
          const T* __restrict__ v0, T* __restrict__ u, int mchunk) {
     pdl_start();
     static_assert(!(INTERP && BOOK), "interpolate+correct is fused on level 0 only");
-    using TL = Visit3Tile<T, NS, BOOK>;
+    static_assert(!(VAR && BOOK), "the variable-coefficient form runs level-0 visits only");
+    using TL = Visit3Tile<T, NS, BOOK, VAR>;
     constexpr int VEC = TL::VEC, RS = TL::RS;
     const int tid = threadIdx.x, px = tid % TL::PX, tr = tid / TL::PX;
     const int NM = g.nz;
@@ -169,6 +212,9 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
     auto eps = [&](int arr, int r) { return reinterpret_cast<T*>(epbase + arr * TL::EP_BYTES + (r * TL::NT + tid) * 16); };
     auto us = [&](int st) { return reinterpret_cast<T*>(epbase + TL::NEP * TL::EP_BYTES + st * TL::UBOX_BYTES); };
     const bool stage_u = !BOOK && u != nullptr;
+    // VAR: rings of the face planes, slot = that of g (order fz, fy, fx: fy is read one row below, fx one element left)
+    unsigned char* fcbase = epbase + TL::NEP * TL::EP_BYTES + (BOOK ? 0 : TL::NU * TL::UBOX_BYTES);
+    auto fcs = [&](int arr, int st) { return reinterpret_cast<T*>(fcbase + (arr * TL::NG + st) * TL::BOX_BYTES); };
     auto buf = [&](int s, int slot) {                              // plane published by stage s
         return reinterpret_cast<T*>(sbase + ((INTERP ? s : s - 1) * 2 + slot) * TL::PLANE_BYTES);
     };
@@ -204,8 +250,14 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
     };
     auto issue_g = [&](int i) {                                    // plane zs+i of g (read at step i+1)
         const int st = i & (TL::NG - 1);
-        mbar_arrive_expect_tx(&gbar[st], TL::BOX_BYTES);
+        mbar_arrive_expect_tx(&gbar[st], (VAR ? 5 : 1) * TL::BOX_BYTES);
         tma_load_3d(gs(st), &tm_g, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
+        if (VAR) {
+            tma_load_3d(fcs(0, st), &tm_fz, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
+            tma_load_3d(fcs(1, st), &tm_fy, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
+            tma_load_3d(fcs(2, st), &tm_fx, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
+            tma_load_3d(fcs(3, st), &tm_wd, &gbar[st], x0 - TL::HX, y0 - TL::HY, zs + i);
+        }
     };
     auto issue_u = [&](int i) {                                    // stored region of u at the plane step i finishes
         const int st = i & (TL::NU - 1);
@@ -307,6 +359,26 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
             for (int s = 0; s < NS - 1; ++s) Gh[s][r].v[j] = T(0);
         }
 
+    // VAR: faces of the plane stage s works on, carried from stage to stage like g (stage s reads the plane stage s-1
+    // read one step earlier): z+ faces of my two rows, y faces of rows ye-1, ye, ye+1, x+ faces of my two rows and
+    // the x- face of each pack's first node; and the z- face of every stage = the z+ face it used one step ago
+    constexpr int NF = VAR ? NS - 1 : 1, NZ = VAR ? NS : 1;
+    Pack<T> Fzh[NF][2], Fyh[NF][3], Fxh[NF][2], Fzm[NZ][2], Wdh[NF][2];
+    T Fxlh[NF][2];
+    if (VAR) {
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) {
+#pragma unroll
+            for (int s = 0; s < NF; ++s) {
+                Fzh[s][0].v[j] = Fzh[s][1].v[j] = Fxh[s][0].v[j] = Fxh[s][1].v[j] = Wdh[s][0].v[j] = Wdh[s][1].v[j] = T(0);
+                Fyh[s][0].v[j] = Fyh[s][1].v[j] = Fyh[s][2].v[j] = T(0);
+                Fxlh[s][0] = Fxlh[s][1] = T(0);
+            }
+#pragma unroll
+            for (int s = 0; s < NZ; ++s) Fzm[s][0].v[j] = Fzm[s][1].v[j] = T(0);
+        }
+    }
+
     // address of (x, ye) in the plane the LAST stage produces at step q: z = zs + q - NS
     long long cF = (long long)(zs - NS) * mstride + (long long)ye * g.px + x;
     const long long rowO = g.px;
@@ -375,6 +447,30 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
 #pragma unroll
             for (int j = 0; j < VEC; ++j) { gn[0].v[j] = T(0); gn[1].v[j] = T(0); }
         }
+        // VAR: the faces of plane z0-1 (same ring slot, same barrier as g)
+        Pack<T> fzn[2], fyn[3], fxn[2], wdn[2];
+        T fxln[2] = {T(0), T(0)};
+        if (VAR) {
+            if (STEADY || q >= 1) {
+                fzn[0] = *reinterpret_cast<const Pack<T>*>(fcs(0, KP) + goffE);
+                fzn[1] = *reinterpret_cast<const Pack<T>*>(fcs(0, KP) + goffO);
+                fyn[0] = *reinterpret_cast<const Pack<T>*>(fcs(1, KP) + goffE - RS);
+                fyn[1] = *reinterpret_cast<const Pack<T>*>(fcs(1, KP) + goffE);
+                fyn[2] = *reinterpret_cast<const Pack<T>*>(fcs(1, KP) + goffO);
+                fxn[0] = *reinterpret_cast<const Pack<T>*>(fcs(2, KP) + goffE);
+                fxn[1] = *reinterpret_cast<const Pack<T>*>(fcs(2, KP) + goffO);
+                wdn[0] = *reinterpret_cast<const Pack<T>*>(fcs(3, KP) + goffE);
+                wdn[1] = *reinterpret_cast<const Pack<T>*>(fcs(3, KP) + goffO);
+                fxln[0] = fcs(2, KP)[goffE - 1];
+                fxln[1] = fcs(2, KP)[goffO - 1];
+            } else {
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) {
+                    fzn[0].v[j] = fzn[1].v[j] = fxn[0].v[j] = fxn[1].v[j] = wdn[0].v[j] = wdn[1].v[j] = T(0);
+                    fyn[0].v[j] = fyn[1].v[j] = fyn[2].v[j] = T(0);
+                }
+            }
+        }
         // y neighbours across threads: row ye-1 (below my even row) and row ye+2 (above my odd row), published in
         // the previous step.  Those of stage s+1 are fetched BEFORE stage s stores (the compiler cannot move a
         // shared load above a shared store by itself).
@@ -403,7 +499,18 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
                 const Pack<T>& gv = s == 1 ? gn[r] : Gh[s == 1 ? 0 : s - 2][r];
                 const T vl = __shfl_up_sync(0xffffffffu, cu.v[VEC - 1], 1);
                 const T vr = __shfl_down_sync(0xffffffffu, cu.v[0], 1);
-                out[r] = jacobi_pack(pv, cu, nx[r], dn, up, gv, vl, vr, wpm[r], cf);
+                if (VAR) {
+                    const Pack<T>& fzp = s == 1 ? fzn[r] : Fzh[s == 1 ? 0 : s - 2][r];
+                    const Pack<T>& fym = s == 1 ? fyn[r] : Fyh[s == 1 ? 0 : s - 2][r];
+                    const Pack<T>& fyp = s == 1 ? fyn[r + 1] : Fyh[s == 1 ? 0 : s - 2][r + 1];
+                    const Pack<T>& fxp = s == 1 ? fxn[r] : Fxh[s == 1 ? 0 : s - 2][r];
+                    const T fxl = s == 1 ? fxln[r] : Fxlh[s == 1 ? 0 : s - 2][r];
+                    const Pack<T>& wdv = s == 1 ? wdn[r] : Wdh[s == 1 ? 0 : s - 2][r];
+                    out[r] = jacobi_pack_var(pv, cu, nx[r], dn, up, gv, vl, vr, wdv, Fzm[s - 1][r], fzp, fym, fyp, fxp, fxl, cf);
+                    Fzm[s - 1][r] = fzp;                          // the z- face of this stage's next plane
+                } else {
+                    out[r] = jacobi_pack(pv, cu, nx[r], dn, up, gv, vl, vr, wpm[r], cf);
+                }
                 if (!zin) {                                        // Dirichlet planes z = 0, nz-1 (and beyond)
 #pragma unroll
                     for (int j = 0; j < VEC; ++j) out[r].v[j] = T(0);
@@ -455,6 +562,19 @@ k_visit3(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUte
 #pragma unroll
         for (int s = NS - 2; s >= 1; --s) { Gh[s][0] = Gh[s - 1][0]; Gh[s][1] = Gh[s - 1][1]; }
         Gh[0][0] = gn[0]; Gh[0][1] = gn[1];
+        if (VAR) {
+#pragma unroll
+            for (int s = NS - 2; s >= 1; --s) {
+                Fzh[s][0] = Fzh[s - 1][0]; Fzh[s][1] = Fzh[s - 1][1]; Fxh[s][0] = Fxh[s - 1][0]; Fxh[s][1] = Fxh[s - 1][1];
+                Fyh[s][0] = Fyh[s - 1][0]; Fyh[s][1] = Fyh[s - 1][1]; Fyh[s][2] = Fyh[s - 1][2];
+                Fxlh[s][0] = Fxlh[s - 1][0]; Fxlh[s][1] = Fxlh[s - 1][1];
+                Wdh[s][0] = Wdh[s - 1][0]; Wdh[s][1] = Wdh[s - 1][1];
+            }
+            Fzh[0][0] = fzn[0]; Fzh[0][1] = fzn[1]; Fxh[0][0] = fxn[0]; Fxh[0][1] = fxn[1];
+            Fyh[0][0] = fyn[0]; Fyh[0][1] = fyn[1]; Fyh[0][2] = fyn[2];
+            Fxlh[0][0] = fxln[0]; Fxlh[0][1] = fxln[1];
+            Wdh[0][0] = wdn[0]; Wdh[0][1] = wdn[1];
+        }
         cF += mstride;
     };
     int q = 0;

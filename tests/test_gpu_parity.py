@@ -650,3 +650,28 @@ def test_brick_and_pack_level_change_kernels_agree_bitwise(orc, monkeypatch):
         for x, y in zip(a, b):
             assert np.array_equal(x, y), (name, n, kw)
         assert np.array_equal(na, nb)
+
+
+@pytest.mark.parametrize("n,kw", [(65, {"tiled_min_nodes": 200000}), (129, {}), (129, {"march_chunk": 20}), (33, {"tiled_min_nodes": 1})])
+def test_variable_coefficient_kvisit_vs_per_sweep_kernels_and_oracle(orc, monkeypatch, n, kw):
+    """K_visit for the variable-coefficient stencil (k_visit3<VAR>: interpolate+correct + 2 sweeps, then
+    2 sweeps + u += e; the face arrays and omega/D staged by TMA once per pass).  It multiplies by the precomputed
+    RN(omega/D) where the per-sweep kernels and the oracle divide (R14): agreement to rounding, not bit for bit
+    — <= 1e-13 against the per-sweep path, <= 1e-12 against the oracle after every cycle (cfg5's recipe)."""
+    cfg = I.scaled(I.CONFIGS["cfg5"], n)
+    inp = I.make_inputs(cfg)
+    ncyc = 6
+    monkeypatch.setenv("HOMG_VISIT_VAR", "1")
+    a, na, _ = run_gpu(cfg, inp, ncyc, **kw)
+    monkeypatch.setenv("HOMG_VISIT_VAR", "0")
+    b, nb, _ = run_gpu(cfg, inp, ncyc, **kw)
+    worst = max(float(np.max(np.abs(x - y)) / np.max(np.abs(y))) for x, y in zip(a, b))
+    assert 0 < worst <= 1e-13, worst                 # (> 0: the fused form really ran)
+    assert np.allclose(na, nb, rtol=1e-9)
+    monkeypatch.setenv("HOMG_VISIT_VAR", "1")
+    check_parity(cfg, ncyc, orc, **kw)
+    if n == 65:                                     # the mixed-precision loop keeps the bit-exact per-sweep kernels
+        us, norms, sched = run_gpu(cfg, inp, 4, mixed=True, **kw)
+        _, hist, onorms = orc.homg_mixed(inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, 4, k=inp["k"])
+        for c in range(4):
+            assert np.max(np.abs(us[c] - hist[c])) <= 1e-12 * np.max(np.abs(hist[c]))
