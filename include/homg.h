@@ -28,6 +28,12 @@
  *     of the last error is available from homg_last_error.
  *   - all device work is issued on the stream given in homg_options.cuda_stream
  *     (NULL = the legacy default stream).
+ *   - environment: HOMG_* variables (HOMG_COARSE_NODES, HOMG_COARSE_CLUSTER, HOMG_COARSE_RELAXN,
+ *     HOMG_TILED_MIN_NODES, HOMG_MARCH_CHUNK, HOMG_PDL, HOMG_FUSE_FIRST, HOMG_FUSE_FIRST_VAR, HOMG_FUSE_VISIT,
+ *     HOMG_VISIT3, HOMG_VISIT_VAR, HOMG_BRICKS, HOMG_DEBUG_SYNC) are read once by homg_create and override the
+ *     corresponding homg_options / defaults.  They select between kernels that compute the same cycle (A/B
+ *     measurements, the bit-for-bit tests of tests/test_gpu_parity.py); a production caller sets none of them.
+ *     HOMG_DEBUG_SYNC synchronises after every launch outside graph capture (to localise a faulting kernel).
  */
 #ifndef HOMG_H_
 #define HOMG_H_
@@ -122,7 +128,9 @@ HOMG_API void homg_default_options(homg_options* opt);
  * arrays plus the fp32 hierarchy (0 on bad arguments). */
 HOMG_API size_t homg_workspace_bytes_mixed(int ndim, const int64_t* dims, int levels, homg_stencil stencil);
 
-/* Bytes of device workspace homg_create needs for this hierarchy (0 on bad arguments).
+/* Bytes of device workspace homg_create needs for this hierarchy (0 on bad arguments), for the default
+ * history_cap of 4096 entries: a caller that asks for a larger homg_options.history_cap adds
+ * (history_cap - 4096) * 8 bytes rounded up to 256 (twice that for a mixed-precision solver).
  * Layout: DESIGN.md "Data layout in HBM" — every level array is contiguous, rows padded
  * to a multiple of 128 bytes, every array 256-byte aligned. */
 HOMG_API size_t homg_workspace_bytes(int ndim, const int64_t* dims, int levels, homg_stencil stencil,
@@ -164,15 +172,18 @@ HOMG_API homg_status homg_cycle(homg_solver* s, int n);
  * HOMG_EINVAL if history_cap < cycles already run + max_cycles + 1. */
 HOMG_API homg_status homg_solve(homg_solver* s, double rel_tol, int max_cycles, int* cycles_done, double* rel_residual);
 
-/* || f - A u ||_2 of the CURRENT u (one norm-only pass, stream sync, 8-byte D2H) and its
+/* PAPER.md L75 ("the residual equation is used to restart the cycles … to reach any desired accuracy"): the accuracy
+ * reached.  || f - A u ||_2 of the CURRENT u (one norm-only pass, stream sync, 8-byte D2H) and its
  * ratio to the first history entry (the norm of the initial guess; 1 if no cycle ran).
  * Either output pointer may be NULL. */
 HOMG_API homg_status homg_residual_norm(homg_solver* s, double* abs_l2, double* rel_to_initial);
 
-/* Copies min(cap, count) history entries (L2 norms, not squared) to host `out`; syncs. */
+/* The residual norms of the restarts so far (the convergence history of the cycles).
+ * Copies min(cap, count) history entries (L2 norms, not squared) to host `out`; syncs. */
 HOMG_API homg_status homg_residual_history(homg_solver* s, double* out, int cap, int* count);
 
-/* Dense C-order copy of u (boundary = 0) into dst; syncs when dst is a host pointer. */
+/* The solution u of A u = f (Eq. 1) after the cycles run so far, Dirichlet u = 0 on the boundary
+ * (L89-93).  Dense C-order copy of u into dst; syncs when dst is a host pointer. */
 HOMG_API homg_status homg_get_solution(homg_solver* s, void* dst, int on_device);
 
 /* Introspection for tests and the bench harness: the effective schedule (returns its
