@@ -28,6 +28,14 @@ struct alignas(2 * sizeof(T)) HalfPack {
     T v[2];
 };
 
+// sm_100a packed fp32 pairs: add / fma .rn.f32x2 (SASS FADD2 / FFMA2) are two IEEE round-to-nearest operations per
+// instruction — the bits of the scalar form at half the issue slots (used by K_visit, 2-D and 3-D)
+struct F2 { unsigned long long b; };
+__device__ __forceinline__ F2 f2_make(float lo, float hi) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.b) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void f2_get(F2 a, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.b)); }
+__device__ __forceinline__ F2 f2_add(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.b) : "l"(a.b), "l"(b.b)); return r; }
+__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.b) : "l"(a.b), "l"(b.b), "l"(c.b)); return r; }
+
 // x / D for a per-level constant D with rD = RN(1/D) precomputed on the host: q = RN(x rD),
 // r = x - q D (exact in one FMA), result RN(q + r rD).  By Markstein's theorem this is the correctly
 // rounded quotient, i.e. bit-identical to the IEEE division the generic kernels and the oracle

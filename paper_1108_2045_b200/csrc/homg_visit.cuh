@@ -63,6 +63,45 @@ struct VisitTile {
     static_assert(PLANE_BYTES % 128 == 0 && BOX_BYTES % 128 == 0 && (BW * ES) % 128 == 0, "TMA destinations are 128-B aligned");
 };
 
+// One Jacobi stage of the 2-D form on a pack (r02): out = v + w_p (((pv + nx) + (xm + xp)) - 4 v) + h^2 g), Eq. 3 in the
+// order of DESIGN.md R14, with the Dirichlet condition as the per-node multiplier w_p in {w/4, 0} (v is 0 there, so
+// v + 0 t = 0) instead of a select.  fp32: packed pairs (FADD2 / FFMA2), the same bits at half the issue slots.
+template <class T>
+__device__ __forceinline__ Pack<T> jacobi_pack2d(const Pack<T>& pv, const Pack<T>& cu, const Pack<T>& nx, const Pack<T>& gv, T vl,
+                                                 T vr, const Pack<T>& wpm, const Coef<T>& cf) {
+    constexpr int VEC = 16 / int(sizeof(T));
+    Pack<T> out;
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+        const T vc = cu.v[j];
+        const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
+        const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+        T sm = pv.v[j] + nx.v[j];
+        sm += xm + xp;
+        T t = fma_rn(-cf.twod, vc, sm);
+        t = fma_rn(cf.h2, gv.v[j], t);
+        out.v[j] = fma_rn(wpm.v[j], t, vc);
+    }
+    return out;
+}
+__device__ __forceinline__ Pack<float> jacobi_pack2d(const Pack<float>& pv, const Pack<float>& cu, const Pack<float>& nx,
+                                                     const Pack<float>& gv, float vl, float vr, const Pack<float>& wpm,
+                                                     const Coef<float>& cf) {
+    const F2 ntd = f2_make(-cf.twod, -cf.twod), h2 = f2_make(cf.h2, cf.h2);
+    const float xs[4] = {vl + cu.v[1], cu.v[0] + cu.v[2], cu.v[1] + cu.v[3], cu.v[2] + vr};
+    Pack<float> out;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const F2 c2 = f2_make(cu.v[2 * h], cu.v[2 * h + 1]);
+        F2 sm = f2_add(f2_make(pv.v[2 * h], pv.v[2 * h + 1]), f2_make(nx.v[2 * h], nx.v[2 * h + 1]));
+        sm = f2_add(sm, f2_make(xs[2 * h], xs[2 * h + 1]));
+        F2 t = f2_fma(ntd, c2, sm);
+        t = f2_fma(h2, f2_make(gv.v[2 * h], gv.v[2 * h + 1]), t);
+        f2_get(f2_fma(f2_make(wpm.v[2 * h], wpm.v[2 * h + 1]), t, c2), out.v[2 * h], out.v[2 * h + 1]);
+    }
+    return out;
+}
+
 template <class T, int ND, int NS, bool INTERP>
 __host__ __device__ constexpr int visit_smem_bytes() {
     using TL = VisitTile<T, ND, NS>;
@@ -171,6 +210,9 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
     bool xin[VEC];
 #pragma unroll
     for (int j = 0; j < VEC; ++j) xin[j] = row_int && (x + j > 0) && (x + j < g.nx - 1);
+    Pack<T> wpm;                                                   // 2-D: Eq. 3's w_p, 0 off the interior
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) wpm.v[j] = xin[j] ? cf.wp : T(0);
     const bool own = px * VEC >= TL::HX && px * VEC < TL::HX + TL::OX && x < g.nx &&
                      (ND == 2 || (py >= TL::HY && py < TL::HY + TL::OY && y < g.ny));
     // INTERP: my first coarse node inside a coarse tile
@@ -223,11 +265,21 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
     };
 
     // register state: own column of every stage input (previous and current plane), g of the stages
+    // g of a plane read once and carried down the stages in registers: measured slower in this kernel (the 12 registers it
+    // costs spill at the 96 that four CTAs per SM leave: level-0 visit of cfg3 259 -> 275 us) — kept switchable, off
+#ifndef HOMG_VISIT2D_G_CHAIN
+#define HOMG_VISIT2D_G_CHAIN 0
+#endif
+    constexpr bool G_CHAIN = ND == 2 && HOMG_VISIT2D_G_CHAIN;
     Pack<T> P[NS], C[NS];
+    Pack<T> Gh[NS - 1];
 #pragma unroll
     for (int s = 0; s < NS; ++s)
 #pragma unroll
-        for (int j = 0; j < VEC; ++j) { P[s].v[j] = T(0); C[s].v[j] = T(0); }
+        for (int j = 0; j < VEC; ++j) {
+            P[s].v[j] = T(0); C[s].v[j] = T(0);
+            if (s < NS - 1) Gh[s].v[j] = T(0);
+        }
 
     // address of (x, y) in the plane the LAST stage produces at step q: z = zs + q - NS
     long long cF = (long long)(zs - NS) * mstride + (ND == 3 ? (long long)y * g.px : 0) + x;
@@ -242,7 +294,11 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
         Pack<T> nx;
         if (INTERP) {
             nx = produce(z0);
-            *reinterpret_cast<Pack<T>*>(buf(0, W) + off) = nx;
+            if (ND == 3) *reinterpret_cast<Pack<T>*>(buf(0, W) + off) = nx;
+            else {                                                 // 2-D: only the x neighbours across warp borders are read back
+                if ((tid & 31) == 0) buf(0, W)[off] = nx.v[0];
+                if ((tid & 31) == 31) buf(0, W)[off + VEC - 1] = nx.v[VEC - 1];
+            }
         } else {
             mbar_wait(&fbar[K], (q / TL::NIN) & 1);
             nx = *reinterpret_cast<const Pack<T>*>(vring(K) + off);
@@ -272,17 +328,19 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
                 if ((tid & 31) == 0) el = ctr[off - 1];
                 if ((tid & 31) == 31) er = ctr[off + VEC];
             }
-            gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
+            if (!G_CHAIN || s == 1) gv = *reinterpret_cast<const Pack<T>*>(gs((q - s) & (TL::NGR - 1)) + goff);
+            else gv = Gh[s - 2 < 0 ? 0 : s - 2];                   // read at stage 1 of an earlier step
         };
         // (3-D: one CTA of 512 threads per SM leaves 128 registers per thread; fetching ahead spills there)
         constexpr bool AHEAD = ND == 2 || !BOOK;
         Pack<T> dnN, upN, gvN;
         T elN = T(0), erN = T(0);
         if (AHEAD) fetch(1, dnN, upN, gvN, elN, erN);
+        Pack<T> g1 = gvN;                                          // 2-D: g of plane z0-1, enters the chain after the stages
 #pragma unroll
         for (int s = 1; s <= NS; ++s) {
             // stage s: plane z0-s of v^s from v^{s-1}: P (z0-s-1), C (z0-s), nx (z0-s+1)
-            if (!AHEAD) fetch(s, dnN, upN, gvN, elN, erN);
+            if (!AHEAD) { fetch(s, dnN, upN, gvN, elN, erN); if (s == 1) g1 = gvN; }
             const Pack<T> dn = dnN, up = upN, gv = gvN;
             const T el = elN, er = erN;
             if (AHEAD && s < NS) fetch(s + 1, dnN, upN, gvN, elN, erN);
@@ -296,21 +354,31 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
             const int z = z0 - s;
             const bool zin = STEADY || (z > 0 && z < NM - 1);
             Pack<T> out;
+            if (ND == 2) {
+                out = jacobi_pack2d(pv, cu, nx, gv, vl, vr, wpm, cf);
+            } else {
 #pragma unroll
-            for (int j = 0; j < VEC; ++j) {
-                const T vc = cu.v[j];
-                const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
-                const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
-                T sm = pv.v[j] + nx.v[j];
-                if (ND == 3) sm += dn.v[j] + up.v[j];
-                sm += xm + xp;
-                out.v[j] = xin[j] ? jacobi_eq3(vc, sm, gv.v[j], cf) : T(0);
+                for (int j = 0; j < VEC; ++j) {
+                    const T vc = cu.v[j];
+                    const T xm = j == 0 ? vl : cu.v[j - 1 < 0 ? 0 : j - 1];
+                    const T xp = j == VEC - 1 ? vr : cu.v[j + 1 > VEC - 1 ? VEC - 1 : j + 1];
+                    T sm = pv.v[j] + nx.v[j];
+                    sm += dn.v[j] + up.v[j];
+                    sm += xm + xp;
+                    out.v[j] = xin[j] ? jacobi_eq3(vc, sm, gv.v[j], cf) : T(0);
+                }
             }
             if (!zin) {                                            // Dirichlet planes z = 0, nz-1 (and beyond)
 #pragma unroll
                 for (int j = 0; j < VEC; ++j) out.v[j] = T(0);
             }
-            if (s < NS) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
+            if (s < NS) {
+                if (ND == 3) *reinterpret_cast<Pack<T>*>(buf(s, W) + off) = out;
+                else {
+                    if ((tid & 31) == 0) buf(s, W)[off] = out.v[0];
+                    if ((tid & 31) == 31) buf(s, W)[off + VEC - 1] = out.v[VEC - 1];
+                }
+            }
             if (BOOK && s == NS - 2 && s >= 1 && o2 != nullptr && own && (STEADY || (q >= 2 * NS - 2 && q <= nsteps - 3)))
                 *reinterpret_cast<Pack<T>*>(o2 + cF + 2 * mstride) = out;
             if (BOOK && s == NS - 1 && s >= 1 && o1 != nullptr && own && (STEADY || (q >= 2 * NS - 1 && q <= nsteps - 2)))
@@ -335,6 +403,11 @@ k_visit(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUten
                 }
             }
             P[s - 1] = cu; C[s - 1] = nx; nx = out;
+        }
+        if (G_CHAIN) {
+#pragma unroll
+            for (int s = NS - 2; s >= 1; --s) Gh[s] = Gh[s - 1];
+            Gh[0] = g1;
         }
         __syncthreads();
         if (tid == 0) {

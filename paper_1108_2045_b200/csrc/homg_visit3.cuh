@@ -108,11 +108,6 @@ __device__ __forceinline__ Pack<T> jacobi_pack(const Pack<T>& pv, const Pack<T>&
 // instruction, so the results are those of the scalar form bit for bit).  A pack is two pairs (v0,v1), (v2,v3) —
 // the register pairs LDS.128 / STS.128 already use; only the x-neighbour sums (vl+v1, v0+v2), (v1+v3, v2+vr) pair
 // nodes differently and are formed by four scalar additions.  18 instructions per pack instead of 32.
-struct F2 { unsigned long long b; };
-__device__ __forceinline__ F2 f2_make(float lo, float hi) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.b) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ void f2_get(F2 a, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.b)); }
-__device__ __forceinline__ F2 f2_add(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.b) : "l"(a.b), "l"(b.b)); return r; }
-__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.b) : "l"(a.b), "l"(b.b), "l"(c.b)); return r; }
 __device__ __forceinline__ Pack<float> jacobi_pack(const Pack<float>& pv, const Pack<float>& cu, const Pack<float>& nx,
                                                    const Pack<float>& dn, const Pack<float>& up, const Pack<float>& gv,
                                                    float vl, float vr, const Pack<float>& wpm, const Coef<float>& cf) {

@@ -675,3 +675,20 @@ def test_variable_coefficient_kvisit_vs_per_sweep_kernels_and_oracle(orc, monkey
         _, hist, onorms = orc.homg_mixed(inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, 4, k=inp["k"])
         for c in range(4):
             assert np.max(np.abs(us[c] - hist[c])) <= 1e-12 * np.max(np.abs(hist[c]))
+
+
+def test_3d_kvisit_forms_agree_bitwise(orc, monkeypatch):
+    """k_visit3 (homg_visit3.cuh, the default) and the 3-D form of k_visit (homg_visit.cuh, HOMG_VISIT3=0: the fallback)
+    run the same visits with different tiles, pipelines and instruction selection (packed pairs, multiplier instead
+    of select): the same bits, level 0 and the bookkeeping form of levels >= 1."""
+    for name, n in (("cfg4", 129), ("cfg2", 65)):
+        cfg = I.scaled(I.CONFIGS[name], n)
+        inp = I.make_inputs(cfg)
+        out = {}
+        for v in ("2", "1", "0"):
+            monkeypatch.setenv("HOMG_VISIT3", v)
+            out[v] = run_gpu(cfg, inp, 2, tiled_min_nodes=200000)
+        for v in ("1", "0"):
+            for x, y in zip(out["2"][0], out[v][0]):
+                assert np.array_equal(x, y), (name, v)
+            assert np.array_equal(out["2"][1], out[v][1])
