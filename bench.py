@@ -134,8 +134,8 @@ def make_solver(cfg, inp, torch, dev, vcycle=None, literal=False, mixed=False):
 
 class Solve:
     """one solve of the workload = one bench step.  MFMG: homg_solve (the device-side loop stops by itself; a config
-    without a tolerance runs its fixed cycle count).  Side rows (classic V, paper-literal, mixed precision) have no
-    homg_solve: they run the cycle count a first run of the same solve needed (find_cstar)."""
+    without a tolerance runs its fixed cycle count; --mixed: the mixed-precision loop, also through homg_solve).  Side
+    rows (classic V, paper-literal) have no homg_solve: they run the cycle count a first run of the same solve needed (find_cstar)."""
 
     def __init__(self, s, cfg, own_loop):
         self.s, self.cfg, self.own_loop, self.cstar = s, cfg, own_loop, None
@@ -304,7 +304,7 @@ def run_homg(args):
         import dataclasses
         cfg = dataclasses.replace(cfg, dtype="f64")
     inp = I.make_inputs(cfg)
-    own_loop = args.cycle == "mfmg" and not args.mixed
+    own_loop = args.cycle == "mfmg"                       # homg_solve: the MFMG cycle, plain or mixed precision
     s, d = make_solver(cfg, inp, torch, dev, vcycle=(2, 1) if args.cycle == "v" else None,
                        literal=args.cycle == "literal", mixed=args.mixed)
     job = Solve(s, cfg, own_loop)

@@ -168,7 +168,7 @@ HOMG_API homg_status homg_cycle(homg_solver* s, int n);
  * is not involved between the launch and the end of the solve (no transfer, no synchronisation inside).  The call
  * then synchronises the stream and reads back the cycle count and two norms (20 bytes).  History: one entry per
  * cycle run (the norm before it), as homg_cycle.  *cycles_done = cycles run by this call, *rel_residual = final
- * || r || / || r_0 || (either may be NULL).  HOMG_CYCLE_MFMG only (not mixed precision): HOMG_ESTATE otherwise.
+ * || r || / || r_0 || (either may be NULL).  HOMG_CYCLE_MFMG only (plain or mixed precision): HOMG_ESTATE otherwise.
  * HOMG_EINVAL if history_cap < cycles already run + max_cycles + 1. */
 HOMG_API homg_status homg_solve(homg_solver* s, double rel_tol, int max_cycles, int* cycles_done, double* rel_residual);
 

@@ -356,8 +356,8 @@ homg_status homg_solve(homg_solver* s, double rel_tol, int max_cycles, int* cycl
     if (!(rel_tol >= 0) || max_cycles < 0) return set_err(s, HOMG_EINVAL, "homg_solve: rel_tol >= 0 and max_cycles >= 0");
     if (!s->have_rhs) return set_err(s, HOMG_ESTATE, "homg_solve before homg_set_rhs");
     if (s->var && !s->have_coef) return set_err(s, HOMG_ESTATE, "homg_solve before homg_set_coefficient");
-    if (s->inner || s->vcycle || s->literal)
-        return set_err(s, HOMG_ESTATE, "homg_solve runs the MFMG cycle (HOMG_CYCLE_MFMG, not mixed precision); use homg_cycle");
+    if (s->vcycle || s->literal)
+        return set_err(s, HOMG_ESTATE, "homg_solve runs the MFMG cycle (HOMG_CYCLE_MFMG, plain or mixed precision); use homg_cycle");
     const long start = s->cycles_issued;
     if (start + max_cycles + 1 > s->hist_cap) return set_err(s, HOMG_EINVAL, "homg_solve: history_cap too small for max_cycles");
     CU(s, exec_prepare(s));

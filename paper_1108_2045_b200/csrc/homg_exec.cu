@@ -1170,12 +1170,18 @@ cudaError_t exec_prepare(homg_solver* s) {
 // Mixed-precision outer cycle (the restart is a defect-correction loop):
 // `s` is the fp64 outer problem (one level: u, f, r), s->inner the fp32 hierarchy.  r = f - A u and its norm
 // in fp64 (K_res), r rounded to fp32 = the inner right-hand side, ONE fp32 HOMG cycle from e = 0, u += e in fp64.
+// cond != 0: the loop body of homg_solve — the fp64 residual and its norm come LAST (of the new u) and set the loop
+// condition; the first kernel of the body carries no PDL attribute (see Rec)
 template <int ND>
-cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st) {
+cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st, unsigned long long cond = 0) {
     homg_solver* in = s->inner;
     Rec R{s, st};
-    if (s->var) rec_norm<double, ND, true>(R, true, true, false);
-    else rec_norm<double, ND, false>(R, true, true, false);
+    auto outer_norm = [&]() {
+        if (s->var) rec_norm<double, ND, true>(R, true, true, false);
+        else rec_norm<double, ND, false>(R, true, true, false);
+    };
+    if (!cond) outer_norm();
+    else R.nopdl_next = true;
     const LevelGeom& go = s->L[0].g;
     const LevelGeom& gi = in->L[0].g;
     // g_0 of the inner hierarchy = fl32(r): the inner cycle's own S1 would compute f_in - A 0 = f_in, so it is skipped
@@ -1192,6 +1198,7 @@ cudaError_t cycle_mixed(homg_solver* s, cudaStream_t st) {
     klaunch(R, k_cvt4<ND, true>, g4, blk(), 0, go, gi, (double*)s->u, (float*)in->u);
     R.check(TAG_OTHER);
     R.acct(0, 2.5, TAG_OTHER);
+    if (cond) { R.cond = cond; outer_norm(); }
     s->launches_per_cycle = R.launches + Ri.launches;
     s->bytes_cycle_all = R.bytes_all + Ri.bytes_all;
     s->bytes_cycle_l0 = R.bytes_l0 + Ri.bytes_l0;
@@ -1225,11 +1232,16 @@ cudaError_t exec_cycle(homg_solver* s, cudaStream_t st) {
 cudaError_t exec_solve_prologue(homg_solver* s, cudaStream_t st, unsigned long long cond) {
     Rec R{s, st};
     R.cond = cond;
+    if (s->inner) {                                  // mixed precision: the fp64 residual of the outer problem (one level)
+        HOMG_DISPATCH(s, rec_norm, R, true, true, false);
+        return R.err;
+    }
     HOMG_DISPATCH(s, rec_norm, R, true, true, true);
     return R.err;
 }
 // homg_solve, loop body: S2..S4 of one cycle, then S1 of the new u
 cudaError_t exec_solve_body(homg_solver* s, cudaStream_t st, unsigned long long cond) {
+    if (s->inner) return s->ndim == 2 ? cycle_mixed<2>(s, st, cond) : cycle_mixed<3>(s, st, cond);
     Rec R{s, st};
     R.cond = cond;
     R.s1_at_end = true;

@@ -692,3 +692,37 @@ def test_3d_kvisit_forms_agree_bitwise(orc, monkeypatch):
             for x, y in zip(out["2"][0], out[v][0]):
                 assert np.array_equal(x, y), (name, v)
             assert np.array_equal(out["2"][1], out[v][1])
+
+
+@pytest.mark.parametrize("name,n,tol", [("cfg2", 65, 1e-10), ("cfg5", 33, 1e-9), ("cfg1", 129, 1e-8)])
+def test_solve_stops_by_itself_in_mixed_precision(orc, name, n, tol):
+    """homg_solve around the mixed-precision outer loop (fp64 residual and norm at the end of every cycle set the loop
+    condition): the oracle's mixed loop needs the same number of cycles, and the cycles issued one by one give the
+    same u bit for bit."""
+    _torch()
+    from paper_1108_2045_b200 import homg
+    cfg = I.CONFIGS[name] if I.CONFIGS[name].dims[0] == n else I.scaled(I.CONFIGS[name], n)
+    inp = I.make_inputs(cfg)
+    cap = 40
+    def mk():
+        s = homg.Solver(cfg.dims, cfg.levels, cfg.stencil, "f64", omega=cfg.omega, max_iters=cfg.max_iters, mixed=True)
+        if inp["k"] is not None:
+            s.set_coefficient(inp["k"])
+        s.set_rhs(inp["f"])
+        s.set_initial_guess(inp["u0"])
+        return s
+    s = mk()
+    done, rel = s.solve(tol, cap)
+    sched = s.schedule()
+    _, _, onorms = orc.homg_mixed(inp["f"], inp["u0"], cfg.levels, cfg.omega, sched, cap, k=inp["k"], keep_history=False)
+    want = next(c for c, v in enumerate(onorms) if v <= tol * onorms[0])
+    assert done == want and 2 <= want < cap and rel <= tol
+    u = s.get_solution().copy()
+    hist = s.residual_history()
+    assert len(hist) == done and np.allclose(hist, onorms[:done], rtol=1e-9)
+    r = mk()
+    r.cycle(done)
+    assert np.array_equal(r.get_solution(), u) and r.residual_history() == hist
+    d2, _ = s.solve(tol, cap)
+    assert d2 == 0
+    s.destroy(); r.destroy()
