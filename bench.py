@@ -165,8 +165,8 @@ class Solve:
 NCU_TRAFFIC = {
     ("cfg4", "visit_l0"): (1.301990e9 + 0.512010e9, "profiles/r02a_ncu_full_cfg4.md"),
     ("cfg4", "residual_l0"): (1.152890e9 + 0.571569e9, "profiles/r01e_ncu_full_cfg4.md (kernel unchanged since)"),
-    ("cfg3", "visit_l0"): (693.390848e6 + 235.526656e6, "profiles/r01e_ncu_full_cfg3.md (kernel unchanged since)"),
-    ("cfg3", "residual_l0"): (548.102656e6 + 302.414592e6, "profiles/r01e_ncu_full_cfg3.md (kernel unchanged since)"),
+    ("cfg3", "visit_l0"): (693.407488e6 + 234.450432e6, "profiles/r02c_ncu_full_cfg3.md"),
+    ("cfg3", "residual_l0"): (548.152832e6 + 302.227200e6, "profiles/r02c_ncu_full_cfg3.md"),
     ("cfg5", "visit_l0"): ((1.005716e9 + 0.127886e9 + 0.759066e9 + 0.125065e9) / 2, "profiles/r02b_ncu_full_cfg5.md (mean of the two passes of a visit)"),
     ("cfg5", "relax_l0"): (687.057920e6 + 121.797120e6, "profiles/r01e_ncu_full_cfg5.md (kernel unchanged since; HOMG_VISIT_VAR=0)"),
     ("cfg5", "relax_l0_last"): (821.715712e6 + 122.345984e6, "profiles/r01e_ncu_full_cfg5.md (kernel unchanged since; HOMG_VISIT_VAR=0)"),
