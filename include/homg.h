@@ -73,7 +73,11 @@ typedef enum {
                            levels <= k.  Four subdomains, coarse points relative to each external corner
                            with the central points just outside every subdomain, same-subdomain
                            interpolation.  Runs the paper's whole-grid iteration (one launch per
-                           iteration over the fine grid, as HOMG_CYCLE_LITERAL), whatever `cycle` says */
+                           iteration over the fine grid, as HOMG_CYCLE_LITERAL), whatever `cycle` says.
+                           max_iters <= 0 means 32 here (the paper's MaxI of L121): under this reading the
+                           contraction per cycle depends on N and MaxI — MaxI = 4: 0.38 at 256^2, 0.84 at
+                           1024^2, > 1 (divergence) from 2048^2 on; MaxI = 32: 0.04-0.08 up to 8192^2
+                           (R19, measured table in section 11) */
 } homg_stencil;
 
 /* MFMG schedule kinds (Fig.1 is missing — DESIGN.md R3).
@@ -88,7 +92,7 @@ enum {
 typedef struct {
     double omega;     /* weighted-Jacobi damping; <= 0: 4/5 (2-D), 6/7 (3-D)             */
     double h;         /* fine mesh width; <= 0: 1/(dims[0]-1)                            */
-    int max_iters;    /* MaxI; <= 0: 4                                    */
+    int max_iters;    /* MaxI; <= 0: 4 (HOMG_POISSON5_POW2: 32)           */
     int schedule;     /* HOMG_SCHED_*                                                    */
     const int* sched_levels; /* HOMG_SCHED_EXPLICIT: level of every visit (host ptr)     */
     const int* sched_iters;  /* HOMG_SCHED_EXPLICIT: iterations of every visit, >= 1     */

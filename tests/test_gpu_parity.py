@@ -610,22 +610,26 @@ def test_pow2_grids(orc, N, dtype, levels, kind, maxi, fkind):
         assert not np.any(np.take(us[-1], [0, -1], axis=ax))
 
 
-def test_pow2_converges_at_a_grid_independent_rate_and_argument_checks():
-    """PAPER.md L85 on the GPU: with the central points the residual contracts by the same factor per cycle on every
-    power-of-two grid (the oracle pin P12f: < 0.30)."""
+def test_pow2_contraction_and_argument_checks():
+    """PAPER.md section 3 on the GPU, reading R19: with the default MaxI of this stencil (32, the paper's L121) a random
+    error contracts by < 0.1 per cycle on every grid; with MaxI = 4 the factor grows with N (the oracle pin P12h) and the
+    iteration diverges at 2048^2 — the documented limitation of the reading, checked here so that it stays documented."""
     _torch()
     from paper_1108_2045_b200 import homg
-    facs = []
-    for N in (64, 256, 1024):
+    def factor(N, maxi):
         k = int(np.log2(N))
-        f = np.ascontiguousarray(I.sine_rhs((N, N)))
-        s = homg.Solver((N, N), k, "poisson5_pow2", "f64", omega=0.8)
-        s.set_rhs(f)
-        s.cycle(8)
-        h = s.residual_history()
-        facs.append(h[7] / h[6])
+        s = homg.Solver((N, N), k, "poisson5_pow2", "f64", omega=0.8, max_iters=maxi)
+        s.set_rhs(np.zeros((N, N)))
+        s.set_initial_guess(np.ascontiguousarray(I.uniform_field((N, N), 7, -1.0, 1.0)))
+        s.cycle(10)
+        h = s.residual_history() + [s.residual_norm()[0]]
+        assert s.schedule()[1][-1] == (32 if maxi <= 0 else min(maxi, 2 ** k))
         s.destroy()
-    assert max(facs) < 0.30 and max(facs) - min(facs) < 0.05, facs
+        return h[10] / h[9]
+    for N in (64, 256, 1024, 2048):
+        assert factor(N, 0) < 0.1
+    f4 = [factor(N, 4) for N in (64, 256, 1024, 2048)]
+    assert f4 == sorted(f4) and f4[0] < 0.26 and 0.7 < f4[2] < 0.95 and f4[3] > 1.0, f4
     with pytest.raises(homg.HomgError):
         homg.Solver((64, 64), 7, "poisson5_pow2", "f64")            # l = 64 > N/2
     with pytest.raises(homg.HomgError):
